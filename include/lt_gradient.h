@@ -1,0 +1,153 @@
+/*
+ * lt_gradient.h -- C ABI of liblt_gradient.so: the lensing-potential gradient (deflection-angle) map of
+ * arXiv 1902.03252 on a regular pixel grid, summed over N dPIE/PIEMD lenses, on one B200 (sm_100a).
+ *
+ * Operation (P:n = PAPER.md line n):
+ *   For every pixel theta = (x_min + i*dx, y_min + j*dx), 0 <= i < nx, 0 <= j < ny:
+ *     gradPsi(theta) = sum_k Rot(+Phi_k) g_k( Rot(-Phi_k) (theta - theta_center,k) )
+ *   -- Algorithm 1, P:191-226 (translate l.3-4, rotate l.5-6, body l.7-9, rotate back l.10-11, sum l.13-14;
+ *   superposition eq. 14-15).  The per-lens body g_k is the dPIE deflection named by
+ *   BASELINE.json:north_star (the paper's own body is the SIE, eq. 21; dPIE is named at P:385):
+ *   PIEMD deflection at rcore minus PIEMD deflection at rcut, times b0*rcut/(rcut-rcore), i.e. the gradient of the
+ *   potential whose convergence is kappa = (b0/2) rcut/(rcut-rcore) [1/sqrt(rcore^2+rho^2) - 1/sqrt(rcut^2+rho^2)],
+ *   rho^2 = x'^2/(1+e)^2 + y'^2/(1-e)^2 in the lens frame (alpha = grad psi, laplace psi = 2 kappa: eq. 2-4).
+ *   Mixed precision: section 3.2-3.3 and section 4: single precision everywhere, then double
+ *   precision inside centre patches and wherever the critical-line criteria eq. 25 / eq. 28
+ *   on the neighbour differences eq. 24 / 27 fire.  Thresholds scale with dx (R11-R16).
+ *
+ * Conventions
+ *   - All pointers named d_* are DEVICE pointers (cudaMalloc / torch CUDA tensors); h_* are HOST pointers.
+ *   - Ownership: the caller owns every buffer.  The library never allocates or frees device memory, never
+ *     synchronises the stream (except the calls marked "synchronises"), and enqueues all work on `cuda_stream`
+ *     (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *   - Output layout: d_out_grad[2*(j*nx+i) + c], c = 0 -> dPsi/dtheta_1, c = 1 -> dPsi/dtheta_2; x (i) fastest.
+ *     Element type: double for LT_FP64 and LT_MIXED (reading R17), float for LT_FP32.  Must be 16-byte aligned.
+ *   - Lens parameters are fp64 in all modes; the per-lens precompute kernel derives the fp32 copies.
+ *   - Errors: every int-returning entry point returns LT_OK (0) or a negative lt_status; nothing throws or aborts.
+ *     Parameter-domain violations (e outside [0,1), rcore <= 0, rcut <= rcore, non-finite) are detected on the
+ *     device by the precompute kernel: the offending lens contributes NaN and lt_last_status() reports it.
+ *   - n_lens == 0 gives a zero map.  Limits: 0 <= n_lens <= LT_MAX_LENSES, 1 <= nx, ny, nx*ny < 2^31.
+ */
+#ifndef LT_GRADIENT_H
+#define LT_GRADIENT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LT_VERSION 100
+#define LT_MAX_LENSES 65536
+
+typedef struct {              /* one dPIE lens; fp64; lengths in arcsec, angle in radians                         */
+  double x, y;                /* centre theta_center (Alg. 1 Require)                                      */
+  double ellipticity;         /* e in [0,1): enters rho^2 = x'^2/(1+e)^2 + y'^2/(1-e)^2 (reading R1)              */
+  double angle;               /* Phi: counter-clockwise angle from the theta_1 axis to the major axis     */
+  double rcore, rcut;         /* 0 < rcore < rcut                                                                 */
+  double b0;                  /* deflection scale (eq. 22 P:183 for its SIS meaning)                              */
+} lt_lens;
+
+typedef enum { LT_FP64 = 0, LT_FP32 = 1, LT_MIXED = 2 } lt_precision;
+
+typedef enum {
+  LT_OK = 0,
+  LT_ERR_NULL_POINTER = -1,
+  LT_ERR_BAD_SIZE = -2,        /* n_lens < 0 or > LT_MAX_LENSES, nx/ny < 1, nx*ny >= 2^31                        */
+  LT_ERR_BAD_GRID = -3,        /* dx <= 0 or non-finite x_min / y_min / dx                                       */
+  LT_ERR_BAD_MODE = -4,
+  LT_ERR_WORKSPACE_TOO_SMALL = -5,
+  LT_ERR_MISALIGNED = -6,      /* d_out_grad or d_workspace not 16-byte aligned                                  */
+  LT_ERR_BAD_MIXED_PARAMS = -7,
+  LT_ERR_CUDA = -8,            /* a launch or runtime call failed; lt_last_cuda_error() has the cudaError_t      */
+  LT_ERR_BAD_LENS_PARAMS = -9  /* reported by lt_last_status only (device-side domain check)                     */
+} lt_status;
+
+typedef struct {               /* mixed-rule constants; lt_mixed_defaults() gives the paper's values             */
+  double m_max;                /* 3.26: eq. 25 fires when |dx - delta_{1,2}| < dx/m_max (R11)            */
+  double c28;                  /* 0.0104/0.03 (eq. 28): fires when |delta_{3,4}| > c28*dx (R11)           */
+  double patch_halfwidth_cluster;   /* 6.0 arcsec = 400/2 px * 0.03" (R14)                                */
+  double patch_halfwidth_galaxy;    /* 0.3 arcsec =  20/2 px * 0.03"                                             */
+  double b0_cluster_threshold;      /* lenses with b0 >= this are cluster-scale (15 arcsec, R15)                 */
+} lt_mixed_params;
+
+typedef struct {               /* filled by lt_mixed_last_stats */
+  long long n_pixels;          /* -1: not recorded (the caller knows nx*ny)                                      */
+  long long n_flagged;         /* pixels recomputed in double precision = patch OR eq.25 OR eq.28                */
+  long long n_patch, n_eq25, n_eq28;   /* pixels with the respective bit set (not exclusive)                     */
+} lt_mixed_stats;
+
+int lt_version(void);
+const char* lt_error_string(int code);
+int lt_last_cuda_error(void);                      /* cudaError_t of the last LT_ERR_CUDA on this thread        */
+void lt_mixed_defaults(lt_mixed_params* out);
+
+/* Bytes of device scratch lt_gradient_grid needs for these sizes (monotone in every argument).  0 on bad sizes. */
+size_t lt_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode);
+
+/*
+ * The hot path.  Enqueues on cuda_stream: the per-lens precompute kernel, the gradient kernel
+ * (a2-a7) in the requested precision and, for LT_MIXED, the patch/flag/compaction kernels (a8) and the fp64
+ * recompute of the flagged pixels (a9).  Asynchronous; returns after the launches.
+ *   d_lenses       device, n_lens lt_lens structs (= a contiguous [n_lens,7] fp64 array); read only
+ *   mixed_or_null  host pointer; NULL = lt_mixed_defaults; ignored unless mode == LT_MIXED
+ *   d_out_grad     device, nx*ny*2 elements (type per mode, see above); fully overwritten
+ *   d_workspace    device, >= lt_workspace_bytes(...) bytes, 16-byte aligned; contents undefined afterwards except
+ *                  what the *_last_* calls below read.  One workspace must not be shared by concurrent calls.
+ */
+int lt_gradient_grid(const lt_lens* d_lenses, int n_lens,
+                     double x_min, double y_min, double dx, int nx, int ny,
+                     lt_precision mode, const lt_mixed_params* mixed_or_null,
+                     void* d_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Gradient at an arbitrary list of points (the a9 kernel exposed; used for sampled parity at full size and for
+ * image positions).  d_points: n_points*2 doubles (theta_1, theta_2 interleaved); d_out: n_points*2 doubles.
+ * fp64 only.  Same workspace rule with nx = ny = 1.
+ */
+int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
+                       double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * The same call with HOST buffers (the end-to-end path of bench.py's `e2e` figure): enqueues, on cuda_stream, the
+ * host->device copy of the n_lens lens structs from h_lenses, lt_gradient_grid, and the device->host copy of the
+ * whole map into h_out_grad (nx*ny*2 elements, type per mode).  Asynchronous with respect to the host only if both
+ * host buffers are pinned; the caller synchronises cuda_stream before reading h_out_grad.  The device staging
+ * buffers for the catalogue and the map are carved from d_workspace, which must hold
+ * lt_host_workspace_bytes(n_lens, nx, ny, mode) bytes (>= lt_workspace_bytes; 0 on bad sizes).
+ */
+size_t lt_host_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode);
+int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens,
+                          double x_min, double y_min, double dx, int nx, int ny,
+                          lt_precision mode, const lt_mixed_params* mixed_or_null,
+                          void* h_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Launch-configuration knobs (process-wide; 0 = the library's default).  ppt64 / ppt32: pixels per thread of the
+ * fp64 (1, 2) and fp32 (1, 2, 4) grid kernels; chunk64 / chunk32: lens records staged in shared memory at a time;
+ * ctas_per_sm: cap on resident CTAs per SM of the persistent grids.  Results do not depend on any of them except
+ * that the fp32 tile centre moves with ppt32.  Returns LT_ERR_BAD_SIZE on a negative value.
+ */
+int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm);
+
+/* After a call on this workspace: LT_OK or LT_ERR_BAD_LENS_PARAMS (first offending lens index in *bad_lens_or_null).
+ * Synchronises cuda_stream. */
+int lt_last_status(const void* d_workspace, void* cuda_stream, int* bad_lens_or_null);
+
+/* After an LT_MIXED call on this workspace: counts of flagged pixels.  Synchronises cuda_stream. */
+int lt_mixed_last_stats(const void* d_workspace, void* cuda_stream, lt_mixed_stats* out);
+
+/* After an LT_MIXED call: copies the per-pixel flag byte map (bit0 patch, bit1 eq.25, bit2 eq.28; nx*ny bytes)
+ * kept in the workspace into d_flags_out (device).  Asynchronous on cuda_stream. */
+int lt_mixed_last_flags(const void* d_workspace, int n_lens, int nx, int ny, unsigned char* d_flags_out,
+                        void* cuda_stream);
+
+/* FMA-chain microbenchmarks used by bench.py to confirm the FP64 / FP32 peaks on the device in the same run
+ * (SURVEY 8(d)): runs `iters` dependent-free FMAs per thread on a full grid; returns achieved FLOP/s in *flops_out
+ * (2 flops per FMA).  Synchronises.  which: 0 = fp64, 1 = fp32. */
+int lt_peak_probe(int which, int iters, double* flops_out, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LT_GRADIENT_H */

@@ -1,0 +1,449 @@
+// lt_api.cu -- C ABI of liblt_gradient.so (include/lt_gradient.h): argument checks, workspace carving, launches.
+// No torch types, no allocation, no synchronisation except where the header says so.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#include "../../include/lt_gradient.h"
+#include "lt_mixed.cuh"
+
+static_assert(sizeof(lt_lens) == sizeof(LtRawLens), "lt_lens and LtRawLens must have the same layout");
+static_assert(sizeof(LtLens<double>) == 128 && sizeof(LtLens<float>) == 64, "lens record sizes");
+
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+
+struct Tuning {
+  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0;
+};
+Tuning g_tuning;
+
+constexpr int kDefaultChunk64 = 256;   // 32 KB of fp64 records per CTA
+constexpr int kDefaultChunk32 = 1024;  // 64 KB of fp32 records per CTA
+constexpr size_t kAlign = 256;
+
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {   // byte offsets into the workspace
+  size_t header, lens64, lens32, flags, sp, list, total;
+};
+
+Layout make_layout(int n_lens, long long n_pix, bool mixed) {
+  Layout L;
+  size_t o = 0;
+  L.header = o; o += sizeof(LtWsHeader);
+  L.lens64 = o; o += align_up((size_t)n_lens * sizeof(LtLens<double>));
+  L.lens32 = o; o += align_up((size_t)n_lens * sizeof(LtLens<float>));
+  L.flags = o;  if (mixed) o += align_up((size_t)n_pix);
+  L.sp = o;     if (mixed) o += align_up((size_t)n_pix * sizeof(float2));
+  L.list = o;   if (mixed) o += align_up((size_t)n_pix * sizeof(unsigned int));
+  L.total = o;
+  return L;
+}
+
+bool sizes_ok(int n_lens, int nx, int ny) {
+  if (n_lens < 0 || n_lens > LT_MAX_LENSES || nx < 1 || ny < 1) return false;
+  return (long long)nx * (long long)ny < (1LL << 31);
+}
+
+int cuda_fail(cudaError_t e) {
+  g_last_cuda_error = (int)e;
+  return LT_ERR_CUDA;
+}
+#define LT_CUDA(call)                                   \
+  do {                                                  \
+    cudaError_t e_ = (call);                            \
+    if (e_ != cudaSuccess) return cuda_fail(e_);        \
+  } while (0)
+
+struct DeviceInfo {
+  int device = -1, sms = 0;
+  size_t smem_optin = 0;
+};
+int device_info(DeviceInfo& d) {
+  static thread_local DeviceInfo cache;
+  int dev = 0;
+  LT_CUDA(cudaGetDevice(&dev));
+  if (cache.device != dev) {
+    int sms = 0, smem = 0;
+    LT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    LT_CUDA(cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    cache.device = dev;
+    cache.sms = sms;
+    cache.smem_optin = (size_t)smem;
+  }
+  d = cache;
+  return LT_OK;
+}
+
+// persistent grid: min(#work groups, resident CTAs) with the smem opt-in set
+template <class K>
+int grid_for(K kernel, size_t smem, long long n_work, const DeviceInfo& d, int& grid) {
+  LT_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int occ = 0;
+  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, LT_THREADS, smem));
+  if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources);
+  if (g_tuning.ctas_per_sm > 0 && g_tuning.ctas_per_sm < occ) occ = g_tuning.ctas_per_sm;
+  long long g = (long long)occ * d.sms;
+  if (g > n_work) g = n_work;
+  if (g < 1) g = 1;
+  grid = (int)g;
+  return LT_OK;
+}
+
+int pick_chunk(int n_lens, int wanted, size_t rec_bytes, const DeviceInfo& d) {
+  int chunk = wanted;
+  const int max_chunk = (int)((d.smem_optin - 1024) / rec_bytes);
+  if (chunk > max_chunk) chunk = max_chunk;
+  if (chunk > n_lens) chunk = n_lens;
+  if (chunk < 1) chunk = 1;
+  return chunk;
+}
+
+// pixels per thread: the largest of the candidates that still gives every SM about two tiles
+int pick_ppt(int wanted, int max_ppt, int nx, int ny, const DeviceInfo& d) {
+  if (wanted == 1 || wanted == 2 || wanted == 4) return wanted <= max_ppt ? wanted : max_ppt;
+  int ppt = max_ppt;
+  while (ppt > 1) {
+    const long long tiles = (long long)((nx + 32 * ppt - 1) / (32 * ppt)) * ((ny + LT_TILE_H - 1) / LT_TILE_H);
+    if (tiles >= 2LL * d.sms) break;
+    ppt >>= 1;
+  }
+  return ppt;
+}
+
+struct GridArgs {
+  int n_lens;
+  double x_min, y_min, dx;
+  int nx, ny;
+};
+
+template <int PPT>
+int launch_f64_ppt(const LtLens<double>* l64, const GridArgs& a, double2* out, const DeviceInfo& d, cudaStream_t st) {
+  const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
+                               sizeof(LtLens<double>), d);
+  const size_t smem = (size_t)chunk * sizeof(LtLens<double>);
+  const int tiles_x = (a.nx + 32 * PPT - 1) / (32 * PPT), tiles_y = (a.ny + LT_TILE_H - 1) / LT_TILE_H;
+  const long long n_tiles = (long long)tiles_x * tiles_y;
+  int grid = 1;
+  const int rc = grid_for(lt_grad_f64_kernel<PPT>, smem, n_tiles, d, grid);
+  if (rc != LT_OK) return rc;
+  lt_grad_f64_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny,
+                                                         tiles_x, (int)n_tiles, out);
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+int launch_f64(const LtLens<double>* l64, const GridArgs& a, double2* out, const DeviceInfo& d, cudaStream_t st) {
+  switch (pick_ppt(g_tuning.ppt64, 2, a.nx, a.ny, d)) {
+    case 1: return launch_f64_ppt<1>(l64, a, out, d, st);
+    default: return launch_f64_ppt<2>(l64, a, out, d, st);
+  }
+}
+
+template <int PPT>
+int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const GridArgs& a, float2* out,
+                   const DeviceInfo& d, cudaStream_t st) {
+  const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
+                               sizeof(LtLens<float>), d);
+  const size_t smem = (size_t)chunk * sizeof(LtLens<float>);
+  const int tiles_x = (a.nx + 32 * PPT - 1) / (32 * PPT), tiles_y = (a.ny + LT_TILE_H - 1) / LT_TILE_H;
+  const long long n_tiles = (long long)tiles_x * tiles_y;
+  int grid = 1;
+  const int rc = grid_for(lt_grad_f32_kernel<PPT>, smem, n_tiles, d, grid);
+  if (rc != LT_OK) return rc;
+  lt_grad_f32_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, l32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
+                                                         a.ny, tiles_x, (int)n_tiles, out);
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const GridArgs& a, float2* out,
+               const DeviceInfo& d, cudaStream_t st) {
+  switch (pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d)) {
+    case 1: return launch_f32_ppt<1>(l64, l32, a, out, d, st);
+    case 2: return launch_f32_ppt<2>(l64, l32, a, out, d, st);
+    default: return launch_f32_ppt<4>(l64, l32, a, out, d, st);
+  }
+}
+
+template <bool FROM_LIST>
+int launch_list(const LtLens<double>* l64, const GridArgs& a, const unsigned int* list, const LtWsHeader* hdr,
+                const double2* points, long long n_points, long long max_work, double2* out, const DeviceInfo& d,
+                cudaStream_t st) {
+  const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
+                               sizeof(LtLens<double>), d);
+  const size_t smem = (size_t)chunk * sizeof(LtLens<double>);
+  int grid = 1;
+  const int rc = grid_for(lt_grad_list_f64_kernel<FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
+  if (rc != LT_OK) return rc;
+  lt_grad_list_f64_kernel<FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
+                                                                    a.nx, list, hdr, points, n_points, out);
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+int check_mixed(const lt_mixed_params& m) {
+  const bool ok = isfinite(m.m_max) && m.m_max > 0 && isfinite(m.c28) && m.c28 >= 0 &&
+                  isfinite(m.patch_halfwidth_cluster) && m.patch_halfwidth_cluster >= 0 &&
+                  isfinite(m.patch_halfwidth_galaxy) && m.patch_halfwidth_galaxy >= 0 &&
+                  !isnan(m.b0_cluster_threshold);
+  return ok ? LT_OK : LT_ERR_BAD_MIXED_PARAMS;
+}
+
+int precompute(const lt_lens* d_lenses, int n_lens, double dx, unsigned char* ws, const Layout& L, cudaStream_t st) {
+  LT_CUDA(cudaMemsetAsync(ws + L.header, 0, sizeof(LtWsHeader), st));
+  const int blocks = n_lens > 0 ? (n_lens + 127) / 128 : 1;
+  lt_precompute_kernel<<<blocks, 128, 0, st>>>(reinterpret_cast<const LtRawLens*>(d_lenses), n_lens, dx,
+                                               reinterpret_cast<LtLens<double>*>(ws + L.lens64),
+                                               reinterpret_cast<LtLens<float>*>(ws + L.lens32),
+                                               reinterpret_cast<LtWsHeader*>(ws + L.header));
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ peak probes
+// Dependent-free FMA chains (8 independent accumulators per thread) to confirm the FP64 / FP32 pipe peaks in the same
+// run as the bench (peak convention of the paper's Table 1: 2 ops x clock x lanes).
+__device__ double lt_probe_sink64;
+__device__ float lt_probe_sink32;
+
+template <class T>
+__global__ void __launch_bounds__(256) lt_probe_kernel(int iters, T seed) {
+  T a0 = seed + (T)threadIdx.x, a1 = a0 + (T)1, a2 = a0 + (T)2, a3 = a0 + (T)3, a4 = a0 + (T)4, a5 = a0 + (T)5,
+    a6 = a0 + (T)6, a7 = a0 + (T)7;
+  const T m = (T)0.999999, c = (T)1e-6;
+  for (int it = 0; it < iters; ++it) {
+    a0 = lt_fma(a0, m, c); a1 = lt_fma(a1, m, c); a2 = lt_fma(a2, m, c); a3 = lt_fma(a3, m, c);
+    a4 = lt_fma(a4, m, c); a5 = lt_fma(a5, m, c); a6 = lt_fma(a6, m, c); a7 = lt_fma(a7, m, c);
+  }
+  const T s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (s == (T)-12345.678) {   // never true: keeps the chains alive without a store on the timed path
+    if (sizeof(T) == 8) lt_probe_sink64 = (double)s; else lt_probe_sink32 = (float)s;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+int lt_version(void) { return LT_VERSION; }
+
+const char* lt_error_string(int code) {
+  switch (code) {
+    case LT_OK: return "ok";
+    case LT_ERR_NULL_POINTER: return "null pointer";
+    case LT_ERR_BAD_SIZE: return "bad size (n_lens, nx, ny or n_points out of range)";
+    case LT_ERR_BAD_GRID: return "bad grid (dx <= 0 or non-finite x_min / y_min / dx)";
+    case LT_ERR_BAD_MODE: return "unknown precision mode";
+    case LT_ERR_WORKSPACE_TOO_SMALL: return "workspace too small (see lt_workspace_bytes)";
+    case LT_ERR_MISALIGNED: return "buffer not 16-byte aligned";
+    case LT_ERR_BAD_MIXED_PARAMS: return "bad mixed-rule parameters";
+    case LT_ERR_CUDA: return "CUDA runtime error (see lt_last_cuda_error)";
+    case LT_ERR_BAD_LENS_PARAMS: return "lens parameters outside the domain (e in [0,1), 0 < rcore < rcut, finite)";
+  }
+  return "unknown error code";
+}
+
+int lt_last_cuda_error(void) { return g_last_cuda_error; }
+
+void lt_mixed_defaults(lt_mixed_params* out) {
+  if (!out) return;
+  out->m_max = 3.26;
+  out->c28 = 0.0104 / 0.03;                /* eq. 28 P:321 over the paper's pixel size P:301 */
+  out->patch_halfwidth_cluster = 6.0;      /* 400/2 px * 0.03" */
+  out->patch_halfwidth_galaxy = 0.3;       /*  20/2 px * 0.03" */
+  out->b0_cluster_threshold = 15.0;        /* R15 */
+}
+
+int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm) {
+  if (ppt64 < 0 || ppt32 < 0 || chunk64 < 0 || chunk32 < 0 || ctas_per_sm < 0) return LT_ERR_BAD_SIZE;
+  g_tuning.ppt64 = ppt64;
+  g_tuning.ppt32 = ppt32;
+  g_tuning.chunk64 = chunk64;
+  g_tuning.chunk32 = chunk32;
+  g_tuning.ctas_per_sm = ctas_per_sm;
+  return LT_OK;
+}
+
+size_t lt_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode) {
+  if (!sizes_ok(n_lens, nx, ny)) return 0;
+  if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return 0;
+  return make_layout(n_lens, (long long)nx * ny, mode == LT_MIXED).total;
+}
+
+int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                     lt_precision mode, const lt_mixed_params* mixed_or_null, void* d_out_grad, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream) {
+  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
+  if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return LT_ERR_BAD_MODE;
+  if (!d_out_grad || !d_workspace || (n_lens > 0 && !d_lenses)) return LT_ERR_NULL_POINTER;
+  if (!(isfinite(x_min) && isfinite(y_min) && isfinite(dx)) || !(dx > 0.0)) return LT_ERR_BAD_GRID;
+  if (((uintptr_t)d_out_grad & 15) || ((uintptr_t)d_workspace & 15)) return LT_ERR_MISALIGNED;
+  const long long n_pix = (long long)nx * ny;
+  const Layout L = make_layout(n_lens, n_pix, mode == LT_MIXED);
+  if (workspace_bytes < L.total) return LT_ERR_WORKSPACE_TOO_SMALL;
+  lt_mixed_params mp;
+  lt_mixed_defaults(&mp);
+  if (mode == LT_MIXED && mixed_or_null) {
+    mp = *mixed_or_null;
+    const int rc = check_mixed(mp);
+    if (rc != LT_OK) return rc;
+  }
+  DeviceInfo dev;
+  int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)d_workspace;
+  LtWsHeader* hdr = reinterpret_cast<LtWsHeader*>(ws + L.header);
+  const LtLens<double>* l64 = reinterpret_cast<const LtLens<double>*>(ws + L.lens64);
+  const LtLens<float>* l32 = reinterpret_cast<const LtLens<float>*>(ws + L.lens32);
+  const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
+
+  rc = precompute(d_lenses, n_lens, dx, ws, L, st);                                   /* a1 */
+  if (rc != LT_OK) return rc;
+  if (mode == LT_FP64) return launch_f64(l64, a, (double2*)d_out_grad, dev, st);      /* a2-a7 */
+  if (mode == LT_FP32) return launch_f32(l64, l32, a, (float2*)d_out_grad, dev, st);
+
+  /* LT_MIXED: single precision everywhere, flag, double precision on the flagged pixels */
+  unsigned char* flags = ws + L.flags;
+  float2* sp = reinterpret_cast<float2*>(ws + L.sp);
+  unsigned int* list = reinterpret_cast<unsigned int*>(ws + L.list);
+  LtMixedDev md;
+  md.fdx = (float)dx;
+  md.t25 = (float)(dx / mp.m_max);
+  md.t28 = (float)(mp.c28 * dx);
+  md.h_cluster = mp.patch_halfwidth_cluster;
+  md.h_galaxy = mp.patch_halfwidth_galaxy;
+  md.b0_cluster = mp.b0_cluster_threshold;
+  LT_CUDA(cudaMemsetAsync(flags, 0, (size_t)n_pix, st));
+  if (n_lens > 0) {
+    lt_patch_kernel<<<n_lens, 256, 0, st>>>(reinterpret_cast<const LtRawLens*>(d_lenses), n_lens, x_min, y_min, dx,
+                                            nx, ny, md, flags);
+    LT_CUDA(cudaGetLastError());
+  }
+  rc = launch_f32(l64, l32, a, sp, dev, st);
+  if (rc != LT_OK) return rc;
+  {
+    long long blocks = (n_pix + 255) / 256;
+    const long long cap = (long long)dev.sms * 16;
+    if (blocks > cap) blocks = cap;
+    lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, (double2*)d_out_grad, list, hdr);   /* a8 */
+    LT_CUDA(cudaGetLastError());
+  }
+  return launch_list<true>(l64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
+}
+
+int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
+                       double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!sizes_ok(n_lens, 1, 1) || n_points < 0) return LT_ERR_BAD_SIZE;
+  if (!d_workspace || (n_lens > 0 && !d_lenses) || (n_points > 0 && (!d_points || !d_out))) return LT_ERR_NULL_POINTER;
+  if (((uintptr_t)d_out & 15) || ((uintptr_t)d_points & 15) || ((uintptr_t)d_workspace & 15)) return LT_ERR_MISALIGNED;
+  const Layout L = make_layout(n_lens, 1, false);
+  if (workspace_bytes < L.total) return LT_ERR_WORKSPACE_TOO_SMALL;
+  DeviceInfo dev;
+  int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)d_workspace;
+  rc = precompute(d_lenses, n_lens, 1.0, ws, L, st);
+  if (rc != LT_OK || n_points == 0) return rc;
+  const GridArgs a{n_lens, 0.0, 0.0, 1.0, 1, 1};
+  return launch_list<false>(reinterpret_cast<const LtLens<double>*>(ws + L.lens64), a, nullptr,
+                            reinterpret_cast<const LtWsHeader*>(ws + L.header),
+                            reinterpret_cast<const double2*>(d_points), n_points, n_points,
+                            reinterpret_cast<double2*>(d_out), dev, st);
+}
+
+size_t lt_host_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode) {
+  const size_t w = lt_workspace_bytes(n_lens, nx, ny, mode);
+  if (w == 0) return 0;
+  const size_t elem = (mode == LT_FP32) ? sizeof(float2) : sizeof(double2);
+  return align_up(w) + align_up((size_t)n_lens * sizeof(lt_lens)) + align_up((size_t)nx * ny * elem);
+}
+
+int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                          lt_precision mode, const lt_mixed_params* mixed_or_null, void* h_out_grad,
+                          void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
+  if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return LT_ERR_BAD_MODE;
+  if (!h_out_grad || !d_workspace || (n_lens > 0 && !h_lenses)) return LT_ERR_NULL_POINTER;
+  if ((uintptr_t)d_workspace & 15) return LT_ERR_MISALIGNED;
+  if (workspace_bytes < lt_host_workspace_bytes(n_lens, nx, ny, mode)) return LT_ERR_WORKSPACE_TOO_SMALL;
+  const size_t w = align_up(lt_workspace_bytes(n_lens, nx, ny, mode));
+  const size_t lens_bytes = (size_t)n_lens * sizeof(lt_lens);
+  const size_t elem = (mode == LT_FP32) ? sizeof(float2) : sizeof(double2);
+  unsigned char* ws = (unsigned char*)d_workspace;
+  lt_lens* d_lenses = reinterpret_cast<lt_lens*>(ws + w);
+  void* d_out = ws + w + align_up(lens_bytes);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (n_lens > 0) LT_CUDA(cudaMemcpyAsync(d_lenses, h_lenses, lens_bytes, cudaMemcpyHostToDevice, st));
+  const int rc = lt_gradient_grid(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out, ws, w, st);
+  if (rc != LT_OK) return rc;
+  LT_CUDA(cudaMemcpyAsync(h_out_grad, d_out, (size_t)nx * ny * elem, cudaMemcpyDeviceToHost, st));
+  return LT_OK;
+}
+
+int lt_last_status(const void* d_workspace, void* cuda_stream, int* bad_lens_or_null) {
+  if (!d_workspace) return LT_ERR_NULL_POINTER;
+  LtWsHeader h;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LT_CUDA(cudaMemcpyAsync(&h, d_workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
+  LT_CUDA(cudaStreamSynchronize(st));
+  if (bad_lens_or_null) *bad_lens_or_null = h.bad_code > 0 ? h.n_lens - h.bad_code : -1;
+  return h.bad_code > 0 ? LT_ERR_BAD_LENS_PARAMS : LT_OK;
+}
+
+int lt_mixed_last_stats(const void* d_workspace, void* cuda_stream, lt_mixed_stats* out) {
+  if (!d_workspace || !out) return LT_ERR_NULL_POINTER;
+  LtWsHeader h;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LT_CUDA(cudaMemcpyAsync(&h, d_workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
+  LT_CUDA(cudaStreamSynchronize(st));
+  out->n_pixels = -1;          /* not recorded in the header: the caller knows nx*ny */
+  out->n_flagged = (long long)h.list_count;
+  out->n_patch = (long long)h.n_patch;
+  out->n_eq25 = (long long)h.n_eq25;
+  out->n_eq28 = (long long)h.n_eq28;
+  return LT_OK;
+}
+
+int lt_mixed_last_flags(const void* d_workspace, int n_lens, int nx, int ny, unsigned char* d_flags_out,
+                        void* cuda_stream) {
+  if (!d_workspace || !d_flags_out) return LT_ERR_NULL_POINTER;
+  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
+  const Layout L = make_layout(n_lens, (long long)nx * ny, true);
+  LT_CUDA(cudaMemcpyAsync(d_flags_out, (const unsigned char*)d_workspace + L.flags, (size_t)nx * ny,
+                          cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+  return LT_OK;
+}
+
+int lt_peak_probe(int which, int iters, double* flops_out, void* cuda_stream) {
+  if (!flops_out) return LT_ERR_NULL_POINTER;
+  if ((which != 0 && which != 1) || iters < 1) return LT_ERR_BAD_SIZE;
+  DeviceInfo dev;
+  const int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaEvent_t e0, e1;
+  LT_CUDA(cudaEventCreate(&e0));
+  LT_CUDA(cudaEventCreate(&e1));
+  const int grid = dev.sms * 8;
+  for (int rep = 0; rep < 2; ++rep) {      /* first pass warms up */
+    LT_CUDA(cudaEventRecord(e0, st));
+    if (which == 0) lt_probe_kernel<double><<<grid, 256, 0, st>>>(iters, 1.0);
+    else lt_probe_kernel<float><<<grid, 256, 0, st>>>(iters, 1.0f);
+    LT_CUDA(cudaGetLastError());
+    LT_CUDA(cudaEventRecord(e1, st));
+    LT_CUDA(cudaEventSynchronize(e1));
+  }
+  float ms = 0.f;
+  LT_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *flops_out = 2.0 * 8.0 * (double)iters * 256.0 * (double)grid / ((double)ms * 1e-3);
+  return LT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,234 @@
+// lt_kernels.cuh -- device kernels of the gradient-map path: per-lens precompute, the fp64 and
+// fp32 grid kernels, and the fp64 list kernel that serves the mixed-precision recompute (a9) and lt_gradient_points.
+//
+// Mapping: data parallelism over pixels only.  A CTA owns tiles of TILE_W x TILE_H
+// pixels (a warp = one row segment, each thread PPT pixels strided by 32 in x so that every store instruction of a
+// warp is one contiguous 512 B / 256 B line), walks the lens catalogue staged in shared memory in chunks (every lane
+// reads the same record: broadcast LDS.128, no bank conflicts), keeps the 2*PPT accumulators in registers for the whole
+// lens loop (Alg. 1 l.13-14) and stores each pixel once.  The grid is persistent: min(#tiles, CTAs/SM * #SM) CTAs
+// stride over the tiles, so a catalogue that fits one chunk is staged once per CTA (fp64).
+#pragma once
+#include <cuda_runtime.h>
+#include "lt_pack.cuh"
+
+#define LT_WARPS_PER_CTA 8
+#define LT_THREADS (32 * LT_WARPS_PER_CTA)
+#define LT_TILE_H LT_WARPS_PER_CTA
+
+struct LtWsHeader {                 // first 256 bytes of the workspace; zeroed at the start of every call
+  int bad_code;                     // max over invalid lenses of (n_lens - k); 0 = all valid
+  int n_lens;
+  unsigned int list_count;          // number of flagged pixels appended to the list (mixed)
+  unsigned int pad0;
+  unsigned long long n_patch, n_eq25, n_eq28;
+  unsigned long long pad1[27];
+};
+static_assert(sizeof(LtWsHeader) == 256, "workspace header is 256 bytes");
+
+// ------------------------------------------------------------------------------------------------ a1: precompute
+__global__ void lt_precompute_kernel(const LtRawLens* __restrict__ raw, int n_lens, double dx,
+                                     LtLens<double>* __restrict__ l64, LtLens<float>* __restrict__ l32,
+                                     LtWsHeader* __restrict__ hdr) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k == 0) hdr->n_lens = n_lens;
+  if (k >= n_lens) return;
+  const LtRawLens r = raw[k];
+  LtLens<double> D;
+  if (lt_lens_valid(r)) {
+    lt_pack_lens(r, dx, D);
+  } else {
+    lt_poison_lens(D);
+    atomicMax(&hdr->bad_code, n_lens - k);
+  }
+  LtLens<float> F;
+  lt_round_lens(D, F);
+  l64[k] = D;
+  l32[k] = F;
+}
+
+// cooperative copy of `count` 16-byte words global -> shared
+__device__ __forceinline__ void lt_copy16(void* dst, const void* src, int count) {
+  uint4* d = reinterpret_cast<uint4*>(dst);
+  const uint4* s = reinterpret_cast<const uint4*>(src);
+  for (int w = threadIdx.x; w < count; w += blockDim.x) d[w] = s[w];
+}
+
+// ------------------------------------------------------------------------------------------------ fp64 grid kernel
+// a2 pixel coordinate (x_min + i*dx, product and sum rounded separately, exactly as the API states it), a3-a6 per
+// lens (lt_interaction), a7 one double2 store per pixel.
+template <int PPT>
+__global__ void __launch_bounds__(LT_THREADS)
+lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, int n_lens, int chunk, double x_min, double y_min,
+                   double dx, int nx, int ny, int tiles_x, int n_tiles, double2* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char lt_smem[];
+  LtLens<double>* sl = reinterpret_cast<LtLens<double>*>(lt_smem);
+  constexpr int TILE_W = 32 * PPT;
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  const bool single = n_lens <= chunk;
+  if (single) {
+    lt_copy16(sl, lens, n_lens * (int)(sizeof(LtLens<double>) / 16));
+    __syncthreads();
+  }
+  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
+    const int j = ty * LT_TILE_H + wrp;
+    const int i0 = tx * TILE_W + lane;
+    const double t2 = __dadd_rn(y_min, __dmul_rn((double)j, dx));
+    double t1[PPT], G1[PPT], G2[PPT];
+#pragma unroll
+    for (int p = 0; p < PPT; ++p) {
+      t1[p] = __dadd_rn(x_min, __dmul_rn((double)(i0 + 32 * p), dx));
+      G1[p] = 0.0;
+      G2[p] = 0.0;
+    }
+    for (int base = 0; base < n_lens; base += chunk) {
+      const int cnt = min(chunk, n_lens - base);
+      if (!single) {
+        __syncthreads();
+        lt_copy16(sl, lens + base, cnt * (int)(sizeof(LtLens<double>) / 16));
+        __syncthreads();
+      }
+#pragma unroll 1
+      for (int k = 0; k < cnt; ++k) {
+        const LtLens<double> L = sl[k];
+        const double d2 = t2 - L.y0;                                // Alg. 1 l.4
+#pragma unroll
+        for (int p = 0; p < PPT; ++p) lt_interaction<double>(t1[p] - L.x0, d2, L, G1[p], G2[p]);  // l.3, l.5-14
+      }
+    }
+    if (j < ny) {
+#pragma unroll
+      for (int p = 0; p < PPT; ++p) {
+        const int i = i0 + 32 * p;
+        if (i < nx) out[(size_t)j * nx + i] = make_double2(G1[p], G2[p]);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ fp32 grid kernel
+// Same mapping.  Coordinates: for every tile and lens the lens-frame position of the TILE CENTRE
+// is formed in fp64 from the fp64 catalogue while the chunk is staged (a few fp64 operations per lens per tile, i.e.
+// per 256*PPT interactions) and rounded to fp32; each pixel adds its small in-tile offset in fp32:
+//   x' = X0 + il*(dx cos) + jl*(dx sin),  y' = Y0 + jl*(dx cos) - il*(dx sin)      (Alg. 1 l.3-6 merged)
+// so the fp32 rounding of the coordinate is relative to the tile size, not to |theta| (the |theta_c|/|dtheta| term of
+// (A.65)).  All per-interaction arithmetic is FP32.
+template <int PPT>
+__global__ void __launch_bounds__(LT_THREADS)
+lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float>* __restrict__ lens32, int n_lens,
+                   int chunk, double x_min, double y_min, double dx, int nx, int ny, int tiles_x, int n_tiles,
+                   float2* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char lt_smem[];
+  LtLens<float>* sl = reinterpret_cast<LtLens<float>*>(lt_smem);
+  constexpr int TILE_W = 32 * PPT;
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  // in-tile offsets from the tile centre, in pixels (exact in fp32)
+  const float jl = (float)wrp - 0.5f * (float)(LT_TILE_H - 1);
+  float il[PPT];
+#pragma unroll
+  for (int p = 0; p < PPT; ++p) il[p] = (float)(lane + 32 * p) - 0.5f * (float)(TILE_W - 1);
+  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
+    const int j = ty * LT_TILE_H + wrp;
+    const int i0 = tx * TILE_W + lane;
+    // tile centre in the sky frame, fp64
+    const double cx = x_min + ((double)(tx * TILE_W) + 0.5 * (double)(TILE_W - 1)) * dx;
+    const double cy = y_min + ((double)(ty * LT_TILE_H) + 0.5 * (double)(LT_TILE_H - 1)) * dx;
+    float G1[PPT], G2[PPT];
+#pragma unroll
+    for (int p = 0; p < PPT; ++p) {
+      G1[p] = 0.f;
+      G2[p] = 0.f;
+    }
+    for (int base = 0; base < n_lens; base += chunk) {
+      const int cnt = min(chunk, n_lens - base);
+      __syncthreads();
+      for (int k = threadIdx.x; k < cnt; k += LT_THREADS) {
+        LtLens<float> F = lens32[base + k];
+        const LtLens<double>& D = lens64[base + k];
+        const double d1 = cx - D.x0, d2 = cy - D.y0, c = D.c, s = D.s;
+        F.x0 = (float)fma(d1, c, d2 * s);
+        F.y0 = (float)fma(d2, c, -(d1 * s));
+        sl[k] = F;
+      }
+      __syncthreads();
+#pragma unroll 1
+      for (int k = 0; k < cnt; ++k) {
+        const LtLens<float> L = sl[k];
+        const float xr = fmaf(jl, L.dxs, L.x0);
+        const float yr = fmaf(jl, L.dxc, L.y0);
+#pragma unroll
+        for (int p = 0; p < PPT; ++p) {
+          const float x = fmaf(il[p], L.dxc, xr);
+          const float y = fmaf(-il[p], L.dxs, yr);
+          float gx, gy;
+          lt_dpie_body<float>(x, y, L, gx, gy);
+          G1[p] = fmaf(gx, L.c, fmaf(-gy, L.s, G1[p]));            // Alg. 1 l.10 + l.13
+          G2[p] = fmaf(gy, L.c, fmaf(gx, L.s, G2[p]));             // Alg. 1 l.11 + l.14
+        }
+      }
+    }
+    if (j < ny) {
+#pragma unroll
+      for (int p = 0; p < PPT; ++p) {
+        const int i = i0 + 32 * p;
+        if (i < nx) out[(size_t)j * nx + i] = make_float2(G1[p], G2[p]);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ fp64 list kernel
+// One pixel per thread, pixels taken from (a) the compacted list of flagged pixel indices of the mixed rule (a9;
+// count read from the workspace header on the device, no host round trip) or (b) an array of arbitrary points.
+// Uses the same lt_interaction in the same lens order as the fp64 grid kernel: identical bits for identical pixels.
+template <bool FROM_LIST>
+__global__ void __launch_bounds__(LT_THREADS)
+lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, int n_lens, int chunk, double x_min, double y_min,
+                        double dx, int nx, const unsigned int* __restrict__ list, const LtWsHeader* __restrict__ hdr,
+                        const double2* __restrict__ points, long long n_points, double2* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char lt_smem[];
+  LtLens<double>* sl = reinterpret_cast<LtLens<double>*>(lt_smem);
+  const long long total = FROM_LIST ? (long long)hdr->list_count : n_points;
+  const bool single = n_lens <= chunk;
+  if (single) {
+    lt_copy16(sl, lens, n_lens * (int)(sizeof(LtLens<double>) / 16));
+    __syncthreads();
+  }
+  const long long n_groups = (total + LT_THREADS - 1) / LT_THREADS;
+  for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
+    const long long t = g * LT_THREADS + threadIdx.x;
+    const bool live = t < total;
+    double t1 = 0.0, t2 = 0.0;
+    size_t dst = 0;
+    if (live) {
+      if (FROM_LIST) {
+        const unsigned int pix = list[t];
+        const int j = (int)(pix / (unsigned int)nx), i = (int)(pix - (unsigned int)j * (unsigned int)nx);
+        t1 = __dadd_rn(x_min, __dmul_rn((double)i, dx));
+        t2 = __dadd_rn(y_min, __dmul_rn((double)j, dx));
+        dst = pix;
+      } else {
+        const double2 pt = points[t];
+        t1 = pt.x;
+        t2 = pt.y;
+        dst = (size_t)t;
+      }
+    }
+    double G1 = 0.0, G2 = 0.0;
+    for (int base = 0; base < n_lens; base += chunk) {
+      const int cnt = min(chunk, n_lens - base);
+      if (!single) {
+        __syncthreads();
+        lt_copy16(sl, lens + base, cnt * (int)(sizeof(LtLens<double>) / 16));
+        __syncthreads();
+      }
+#pragma unroll 1
+      for (int k = 0; k < cnt; ++k) {
+        const LtLens<double> L = sl[k];
+        lt_interaction<double>(t1 - L.x0, t2 - L.y0, L, G1, G2);
+      }
+    }
+    if (live) out[dst] = make_double2(G1, G2);
+  }
+}

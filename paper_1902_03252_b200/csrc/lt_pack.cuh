@@ -1,0 +1,74 @@
+// lt_pack.cuh -- per-lens precompute: raw (xc, yc, e, Phi, rcore, rcut, b0) -> the packed
+// constants of lt_math.cuh's LtLens<T> record.  All derivations in fp64; the fp32 record is the fp64 one rounded once.
+// P:228 / Fig. 2-3: homogeneous per-parameter data so that every lane reads the same constants;
+// cos/sin of Phi are used four times per interaction in Alg. 1 l.5-6, 10-11 and are taken once here.
+// Host-compilable like lt_math.cuh.
+#pragma once
+#include "lt_math.cuh"
+
+struct LtRawLens {  // = lt_lens of include/lt_gradient.h (kept separate so this header needs no C-ABI include)
+  double x, y, e, phi, rcore, rcut, b0;
+};
+
+// Domain check of the API (include/lt_gradient.h): e in [0,1), 0 < rcore < rcut, everything finite.
+LT_HD bool lt_lens_valid(const LtRawLens& r) {
+  const bool fin = isfinite(r.x) && isfinite(r.y) && isfinite(r.e) && isfinite(r.phi) && isfinite(r.rcore) &&
+                   isfinite(r.rcut) && isfinite(r.b0);
+  return fin && r.e >= 0.0 && r.e < 1.0 && r.rcore > 0.0 && r.rcut > r.rcore;
+}
+
+// fp64 record.  x0, y0 = lens centre; dxc, dxs = dx cos Phi, dx sin Phi.
+LT_HD void lt_pack_lens(const LtRawLens& r, double dx, LtLens<double>& L) {
+  double s, c;
+  sincos(r.phi, &s, &c);
+  const double e = r.e;
+  const double ope = 1.0 + e, ome = 1.0 - e;
+  const double q = ome / ope;
+  const double q2 = q * q;
+  double f = 2.0 * sqrt(e) / ope;            // sqrt(1 - q^2)
+  f = f < LT_F_MIN ? LT_F_MIN : f;           // e = 0 stays a regular point (header of lt_math.cuh)
+  const double sc = r.rcore * ope, st = r.rcut * ope;
+  L.x0 = r.x;
+  L.y0 = r.y;
+  L.c = c;
+  L.s = s;
+  L.dxc = dx * c;
+  L.dxs = dx * s;
+  L.q2 = q2;
+  L.Kc = (ome * r.rcore) * (ome * r.rcore);  // q^2 s_c^2
+  L.Kt = (ome * r.rcut) * (ome * r.rcut);
+  L.sc = sc;
+  L.st = st;
+  L.q2sc = q2 * sc;
+  L.q2st = q2 * st;
+  L.f = f;
+  L.C = r.b0 * (r.rcut / (r.rcut - r.rcore)) * ome / f;
+  L.pad = 0.0;
+}
+
+LT_HD void lt_poison_lens(LtLens<double>& L) {  // invalid parameters: the lens contributes NaN everywhere
+  const double n = NAN;
+  L.x0 = L.y0 = L.c = L.s = L.dxc = L.dxs = L.q2 = L.Kc = L.Kt = L.sc = L.st = L.q2sc = L.q2st = L.f = L.C = n;
+  L.pad = 0.0;
+}
+
+// fp32 record = fp64 record rounded once, except x0, y0 which the fp32 kernel fills per pixel tile (lens-frame
+// coordinates of the tile origin, formed in fp64 and then rounded: DESIGN.md section 5, "fp32 coordinates").
+LT_HD void lt_round_lens(const LtLens<double>& D, LtLens<float>& F) {
+  F.x0 = 0.f;
+  F.y0 = 0.f;
+  F.c = (float)D.c;
+  F.s = (float)D.s;
+  F.dxc = (float)D.dxc;
+  F.dxs = (float)D.dxs;
+  F.q2 = (float)D.q2;
+  F.Kc = (float)D.Kc;
+  F.Kt = (float)D.Kt;
+  F.sc = (float)D.sc;
+  F.st = (float)D.st;
+  F.q2sc = (float)D.q2sc;
+  F.q2st = (float)D.q2st;
+  F.f = (float)D.f;
+  F.C = (float)D.C;
+  F.pad = 0.f;
+}

@@ -1,0 +1,228 @@
+"""Thin Python binding of liblt_gradient.so (include/lt_gradient.h): argument marshalling only.
+
+Every step of the path (per-lens precompute, gradient kernels, mixed-rule flagging, fp64 recompute) runs in the CUDA
+library; PyTorch is used here for device memory and streams.  There is NO CPU fallback: if the shared library is
+missing or cannot be loaded this module raises (it never imports anything from oracle/).
+
+Functions carry the C names; tensors stand for the pointers:
+    lt_gradient_grid(lenses[n,7] f64 cuda, x_min, y_min, dx, nx, ny, mode, ...) -> out [ny, nx, 2]
+"""
+import ctypes
+import os
+
+import torch
+
+LT_FP64, LT_FP32, LT_MIXED = 0, 1, 2
+LT_OK = 0
+LT_ERR_BAD_LENS_PARAMS = -9
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
+
+SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
+           "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
+           "lt_set_tuning", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
+
+
+class lt_mixed_params(ctypes.Structure):
+    _fields_ = [("m_max", ctypes.c_double), ("c28", ctypes.c_double), ("patch_halfwidth_cluster", ctypes.c_double),
+                ("patch_halfwidth_galaxy", ctypes.c_double), ("b0_cluster_threshold", ctypes.c_double)]
+
+
+class lt_mixed_stats(ctypes.Structure):
+    _fields_ = [("n_pixels", ctypes.c_longlong), ("n_flagged", ctypes.c_longlong), ("n_patch", ctypes.c_longlong),
+                ("n_eq25", ctypes.c_longlong), ("n_eq28", ctypes.c_longlong)]
+
+
+class LtError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = lib().lt_error_string(code).decode()
+        if code == -8:
+            msg += " [cudaError %d]" % lib().lt_last_cuda_error()
+        super().__init__("%s: %s (%d)" % (where, msg, code))
+
+
+_lib = None
+
+
+def lib():
+    """Loads the in-tree liblt_gradient.so (built by paper_1902_03252_b200.csrc.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError("liblt_gradient.so is not built: run `python -m paper_1902_03252_b200.csrc.build` "
+                               "(or __graft_entry__.build()).  There is no CPU fallback.")
+        L = ctypes.CDLL(_LIB_PATH)
+        vp, ci, cd, cll, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_longlong, ctypes.c_size_t
+        L.lt_version.restype = ci
+        L.lt_error_string.restype = ctypes.c_char_p
+        L.lt_error_string.argtypes = [ci]
+        L.lt_last_cuda_error.restype = ci
+        L.lt_mixed_defaults.argtypes = [ctypes.POINTER(lt_mixed_params)]
+        L.lt_mixed_defaults.restype = None
+        L.lt_workspace_bytes.argtypes = [ci, ci, ci, ci]
+        L.lt_workspace_bytes.restype = sz
+        L.lt_host_workspace_bytes.argtypes = [ci, ci, ci, ci]
+        L.lt_host_workspace_bytes.restype = sz
+        L.lt_gradient_grid.argtypes = [vp, ci, cd, cd, cd, ci, ci, ci, ctypes.POINTER(lt_mixed_params), vp, vp, sz, vp]
+        L.lt_gradient_grid.restype = ci
+        L.lt_gradient_grid_host.argtypes = L.lt_gradient_grid.argtypes
+        L.lt_gradient_grid_host.restype = ci
+        L.lt_gradient_points.argtypes = [vp, ci, vp, cll, vp, vp, sz, vp]
+        L.lt_gradient_points.restype = ci
+        L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci]
+        L.lt_set_tuning.restype = ci
+        L.lt_last_status.argtypes = [vp, vp, ctypes.POINTER(ci)]
+        L.lt_last_status.restype = ci
+        L.lt_mixed_last_stats.argtypes = [vp, vp, ctypes.POINTER(lt_mixed_stats)]
+        L.lt_mixed_last_stats.restype = ci
+        L.lt_mixed_last_flags.argtypes = [vp, ci, ci, ci, vp, vp]
+        L.lt_mixed_last_flags.restype = ci
+        L.lt_peak_probe.argtypes = [ci, ci, ctypes.POINTER(cd), vp]
+        L.lt_peak_probe.restype = ci
+        _lib = L
+    return _lib
+
+
+def _check(rc, where):
+    if rc != LT_OK:
+        raise LtError(rc, where)
+
+
+def _stream(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _lenses_dev(lenses):
+    if not (isinstance(lenses, torch.Tensor) and lenses.is_cuda and lenses.dtype == torch.float64):
+        raise TypeError("lenses must be a CUDA float64 tensor [n_lens, 7]")
+    lenses = lenses.reshape(-1, 7)
+    if not lenses.is_contiguous():
+        lenses = lenses.contiguous()
+    return lenses
+
+
+def _mixed_ptr(mixed):
+    if mixed is None:
+        return None
+    if isinstance(mixed, lt_mixed_params):
+        return ctypes.byref(mixed)
+    return ctypes.byref(lt_mixed_params(*[float(v) for v in mixed]))
+
+
+def lt_version():
+    return int(lib().lt_version())
+
+
+def lt_mixed_defaults():
+    p = lt_mixed_params()
+    lib().lt_mixed_defaults(ctypes.byref(p))
+    return p
+
+
+def lt_workspace_bytes(n_lens, nx, ny, mode):
+    return int(lib().lt_workspace_bytes(int(n_lens), int(nx), int(ny), int(mode)))
+
+
+def lt_host_workspace_bytes(n_lens, nx, ny, mode):
+    return int(lib().lt_host_workspace_bytes(int(n_lens), int(nx), int(ny), int(mode)))
+
+
+def lt_set_tuning(ppt64=0, ppt32=0, chunk64=0, chunk32=0, ctas_per_sm=0):
+    _check(lib().lt_set_tuning(int(ppt64), int(ppt32), int(chunk64), int(chunk32), int(ctas_per_sm)), "lt_set_tuning")
+
+
+def alloc_workspace(n_lens, nx, ny, mode, device="cuda", host=False):
+    n = (lt_host_workspace_bytes if host else lt_workspace_bytes)(n_lens, nx, ny, mode)
+    if n == 0:
+        raise LtError(-2, "lt_workspace_bytes")
+    return torch.empty(n, dtype=torch.uint8, device=device)
+
+
+def lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None, out=None, workspace=None,
+                     stream=None):
+    """Deflection map on the device.  Returns `out` ([ny, nx, 2]; float32 for LT_FP32, else float64).  Asynchronous."""
+    lenses = _lenses_dev(lenses)
+    n_lens = lenses.shape[0]
+    dt = torch.float32 if mode == LT_FP32 else torch.float64
+    if out is None:
+        out = torch.empty((ny, nx, 2), dtype=dt, device=lenses.device)
+    elif out.dtype != dt or out.numel() != nx * ny * 2 or not out.is_contiguous() or not out.is_cuda:
+        raise TypeError("out must be a contiguous CUDA %s tensor with nx*ny*2 elements" % dt)
+    if workspace is None:
+        workspace = alloc_workspace(n_lens, nx, ny, mode, lenses.device)
+    rc = lib().lt_gradient_grid(ctypes.c_void_p(lenses.data_ptr() if n_lens else None), n_lens, float(x_min),
+                                float(y_min), float(dx), int(nx), int(ny), int(mode), _mixed_ptr(mixed),
+                                ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
+                                workspace.numel(), _stream(stream))
+    _check(rc, "lt_gradient_grid")
+    return out
+
+
+def lt_gradient_grid_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, workspace, mixed=None, stream=None):
+    """End-to-end call with HOST buffers (CPU tensors, ideally pinned): H2D of the catalogue, the hot path, D2H of the
+    map, all enqueued on the stream.  The caller synchronises before reading h_out."""
+    if h_lenses.is_cuda or h_out.is_cuda or h_lenses.dtype != torch.float64 or not h_lenses.is_contiguous():
+        raise TypeError("h_lenses / h_out must be contiguous CPU tensors (float64 catalogue)")
+    n_lens = h_lenses.reshape(-1, 7).shape[0]
+    dt = torch.float32 if mode == LT_FP32 else torch.float64
+    if h_out.dtype != dt or h_out.numel() != nx * ny * 2 or not h_out.is_contiguous():
+        raise TypeError("h_out must be a contiguous CPU %s tensor with nx*ny*2 elements" % dt)
+    rc = lib().lt_gradient_grid_host(ctypes.c_void_p(h_lenses.data_ptr() if n_lens else None), n_lens, float(x_min),
+                                     float(y_min), float(dx), int(nx), int(ny), int(mode), _mixed_ptr(mixed),
+                                     ctypes.c_void_p(h_out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
+                                     workspace.numel(), _stream(stream))
+    _check(rc, "lt_gradient_grid_host")
+    return h_out
+
+
+def lt_gradient_points(lenses, points, out=None, workspace=None, stream=None):
+    """fp64 deflection at arbitrary points ([n, 2] float64 CUDA).  Returns [n, 2]."""
+    lenses = _lenses_dev(lenses)
+    n_lens = lenses.shape[0]
+    if not (points.is_cuda and points.dtype == torch.float64):
+        raise TypeError("points must be a CUDA float64 tensor [n, 2]")
+    points = points.reshape(-1, 2).contiguous()
+    n = points.shape[0]
+    if out is None:
+        out = torch.empty((n, 2), dtype=torch.float64, device=points.device)
+    if workspace is None:
+        workspace = alloc_workspace(n_lens, 1, 1, LT_FP64, points.device)
+    rc = lib().lt_gradient_points(ctypes.c_void_p(lenses.data_ptr() if n_lens else None), n_lens,
+                                  ctypes.c_void_p(points.data_ptr() if n else None), n,
+                                  ctypes.c_void_p(out.data_ptr() if n else None),
+                                  ctypes.c_void_p(workspace.data_ptr()), workspace.numel(), _stream(stream))
+    _check(rc, "lt_gradient_points")
+    return out
+
+
+def lt_last_status(workspace, stream=None):
+    """(code, first offending lens index or -1).  Synchronises the stream."""
+    bad = ctypes.c_int(-1)
+    rc = lib().lt_last_status(ctypes.c_void_p(workspace.data_ptr()), _stream(stream), ctypes.byref(bad))
+    if rc not in (LT_OK, LT_ERR_BAD_LENS_PARAMS):
+        raise LtError(rc, "lt_last_status")
+    return rc, bad.value
+
+
+def lt_mixed_last_stats(workspace, stream=None):
+    s = lt_mixed_stats()
+    _check(lib().lt_mixed_last_stats(ctypes.c_void_p(workspace.data_ptr()), _stream(stream), ctypes.byref(s)),
+           "lt_mixed_last_stats")
+    return {"n_flagged": s.n_flagged, "n_patch": s.n_patch, "n_eq25": s.n_eq25, "n_eq28": s.n_eq28}
+
+
+def lt_mixed_last_flags(workspace, n_lens, nx, ny, stream=None):
+    out = torch.empty((ny, nx), dtype=torch.uint8, device=workspace.device)
+    _check(lib().lt_mixed_last_flags(ctypes.c_void_p(workspace.data_ptr()), int(n_lens), int(nx), int(ny),
+                                     ctypes.c_void_p(out.data_ptr()), _stream(stream)), "lt_mixed_last_flags")
+    return out
+
+
+def lt_peak_probe(which, iters=1 << 16, stream=None):
+    """Achieved FLOP/s of a dependent-free FMA-chain kernel (0 = fp64, 1 = fp32).  Synchronises."""
+    v = ctypes.c_double(0.0)
+    _check(lib().lt_peak_probe(int(which), int(iters), ctypes.byref(v), _stream(stream)), "lt_peak_probe")
+    return v.value

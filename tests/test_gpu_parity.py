@@ -1,0 +1,210 @@
+"""GPU-vs-oracle parity through the C ABI (python binding = marshalling only).  Run on the B200 box: pytest -m gpu.
+
+Metric (R9): per component, max over pixels of |GPU - oracle| / max over pixels of |alpha_oracle|.
+Tolerances: fp64 1e-12 (north star); fp32 1e-5 (north star's example, = the SP accuracy the
+paper deems sufficient away from the DP set); mixed: flagged pixels bit-equal to the fp64 mode and <= 1e-12 of the
+oracle, unflagged pixels == fp32 mode widened.
+"""
+import numpy as np
+import pytest
+
+from paper_1902_03252_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL_F64 = 1e-12
+TOL_F32 = 1e-5
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    from paper_1902_03252_b200 import lt
+    from oracle import lt_oracle as O
+    lt.lib()
+    return torch, lt, O
+
+
+def _gpu_map(torch, lt, W, mode, mixed=None, nx=None, ny=None, ws_out=None):
+    nx = W.nx if nx is None else nx
+    ny = W.ny if ny is None else ny
+    L = torch.from_numpy(W.lenses).cuda()
+    ws = lt.alloc_workspace(L.shape[0], nx, ny, mode)
+    out = lt.lt_gradient_grid(L, W.x_min, W.y_min, W.dx, nx, ny, mode, mixed=mixed, workspace=ws)
+    torch.cuda.synchronize()
+    rc, bad = lt.lt_last_status(ws)
+    assert rc == 0, (rc, bad)
+    if ws_out is not None:
+        ws_out.append(ws)
+    return out.cpu().numpy()
+
+
+def _err(a, ref):
+    s = np.abs(ref).reshape(-1, 2).max(axis=0)
+    return (np.abs(a.astype(np.float64) - ref).reshape(-1, 2).max(axis=0) / s).max()
+
+
+def test_cfg0_fp64_fp32_full_grid(env):
+    torch, lt, O = env
+    W = workloads.make(0)
+    ref = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny)
+    assert _err(_gpu_map(torch, lt, W, lt.LT_FP64), ref) < TOL_F64
+    assert _err(_gpu_map(torch, lt, W, lt.LT_FP32), ref) < TOL_F32
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 200), (2, 136), (4, 2048)])
+def test_reduced_grids_span_tiles_and_ragged_tail(env, cfg, n):
+    """Catalogues of configs 1, 2 (coarser grid of the same extent: several tiles, ragged tails in x and y) and the
+    stress config 4 on a window of its full-resolution grid around lens centres."""
+    torch, lt, O = env
+    W = workloads.make(cfg, n_override=n if cfg != 4 else None)
+    if cfg == 4:
+        # 300 x 77 window of the 2048^2 grid whose lower-left corner sits 20 px left/below lens 5's nearest pixel
+        i0 = int(round((W.lenses[5, 0] - W.x_min) / W.dx)) - 20
+        j0 = int(round((W.lenses[5, 1] - W.y_min) / W.dx)) - 20
+        W = W._replace(x_min=W.x_min + i0 * W.dx, y_min=W.y_min + j0 * W.dx, nx=300, ny=77)
+    else:
+        W = W._replace(nx=n, ny=n - 3)
+    ref = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny)
+    e64 = _err(_gpu_map(torch, lt, W, lt.LT_FP64), ref)
+    e32 = _err(_gpu_map(torch, lt, W, lt.LT_FP32), ref)
+    print("cfg", cfg, "fp64 err", e64, "fp32 err", e32)
+    assert e64 < TOL_F64
+    assert e32 < TOL_F32
+
+
+@pytest.mark.parametrize("ppt64,ppt32,chunk", [(1, 1, 0), (2, 2, 3), (2, 4, 64), (1, 4, 1)])
+def test_launch_configurations_agree(env, ppt64, ppt32, chunk):
+    """Every pixels-per-thread / lens-chunk variant gives the same fp64 bits and fp32 within tolerance."""
+    torch, lt, O = env
+    W = workloads.make(1, n_override=97)
+    ref = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny)
+    base = _gpu_map(torch, lt, W, lt.LT_FP64)
+    try:
+        lt.lt_set_tuning(ppt64, ppt32, chunk, chunk, 0)
+        a = _gpu_map(torch, lt, W, lt.LT_FP64)
+        b = _gpu_map(torch, lt, W, lt.LT_FP32)
+    finally:
+        lt.lt_set_tuning()
+    assert np.array_equal(a, base)
+    assert _err(a, ref) < TOL_F64 and _err(b, ref) < TOL_F32
+
+
+def test_full_size_cfg1_sampled_and_points(env):
+    """BASELINE config 1 at full size, in the launch configuration bench.py times: sampled pixels (random + the pixels
+    nearest every lens centre) against the oracle, and lt_gradient_points against the grid kernel (bit-equal)."""
+    torch, lt, O = env
+    W = workloads.make(1)
+    g64 = _gpu_map(torch, lt, W, lt.LT_FP64)
+    g32 = _gpu_map(torch, lt, W, lt.LT_FP32)
+    rng = np.random.default_rng(42)
+    i = rng.integers(0, W.nx, 20000)
+    j = rng.integers(0, W.ny, 20000)
+    ic = np.clip(np.round((W.lenses[:, 0] - W.x_min) / W.dx), 0, W.nx - 1).astype(np.int64)
+    jc = np.clip(np.round((W.lenses[:, 1] - W.y_min) / W.dx), 0, W.ny - 1).astype(np.int64)
+    i = np.concatenate([i, ic, np.clip(ic + 1, 0, W.nx - 1), [0, W.nx - 1]])
+    j = np.concatenate([j, jc, jc, [0, W.ny - 1]])
+    px, py = W.x_min + i * W.dx, W.y_min + j * W.dx
+    ref = O.gradient_points(W.lenses, px, py)
+    s = np.abs(ref).max(axis=0)
+    assert (np.abs(g64[j, i] - ref).max(axis=0) / s).max() < TOL_F64
+    assert (np.abs(g32[j, i].astype(np.float64) - ref).max(axis=0) / s).max() < TOL_F32
+    pts = torch.from_numpy(np.stack([px, py], axis=1)).cuda()
+    gp = lt.lt_gradient_points(torch.from_numpy(W.lenses).cuda(), pts).cpu().numpy()
+    assert np.array_equal(gp, g64[j, i])
+    # the whole fp32 map against the (now oracle-checked) fp64 map
+    assert _err(g32, g64) < TOL_F32
+
+
+def test_mixed_mode_follows_the_rule(env):
+    """Mixed mode on config 0 and on the paper-regime variant of config 1 (reduced grid): the flag mask equals the
+    oracle's rule applied to the GPU's own fp32 map (bit-exact: both take the fp32 decisions in fp32), flagged pixels
+    carry the fp64 kernel's bits, unflagged pixels the fp32 kernel's value widened; the stats agree with the mask."""
+    torch, lt, O = env
+    for W in (workloads.make(0), workloads.make(1, paper_regime=True, n_override=333)):
+        ws = []
+        m = _gpu_map(torch, lt, W, lt.LT_MIXED, ws_out=ws)
+        g64 = _gpu_map(torch, lt, W, lt.LT_FP64)
+        g32 = _gpu_map(torch, lt, W, lt.LT_FP32)
+        flags = lt.lt_mixed_last_flags(ws[0], len(W.lenses), W.nx, W.ny).cpu().numpy()
+        expect = O.mixed_flags(g32, W.lenses, W.x_min, W.y_min, W.dx)
+        assert np.array_equal(flags, expect)
+        st = lt.lt_mixed_last_stats(ws[0])
+        assert st["n_flagged"] == int((flags != 0).sum())
+        assert st["n_patch"] == int((flags & 1).astype(bool).sum())
+        assert st["n_eq25"] == int((flags & 2).astype(bool).sum())
+        assert st["n_eq28"] == int((flags & 4).astype(bool).sum())
+        f = flags != 0
+        assert np.array_equal(m[f], g64[f])
+        assert np.array_equal(m[~f], g32[~f].astype(np.float64))
+        ref = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny)
+        s = np.abs(ref).max()
+        if f.any():
+            assert np.abs(m[f] - ref[f]).max() / s < TOL_F64
+        assert np.abs(m - ref).max() / s < TOL_F32
+        # the paper's sufficiency criterion: |err| <= dx / (4 M) with M <= m_max on unflagged pixels
+        assert np.abs(m[~f] - ref[~f]).max() <= W.dx / 4 / 3.26 if (~f).any() else True
+        print(W.name, "flagged fraction", f.mean(), st)
+
+
+def test_edge_cases(env):
+    torch, lt, O = env
+    W = workloads.make(0)
+    # n_lens = 0 -> zero map in every mode
+    Z = W._replace(lenses=np.zeros((0, 7)))
+    for mode in (lt.LT_FP64, lt.LT_FP32, lt.LT_MIXED):
+        assert np.all(_gpu_map(torch, lt, Z, mode) == 0)
+    # 1 x 1, 1 x n, n x 1 grids
+    for nx, ny in ((1, 1), (1, 50), (70, 1), (33, 9)):
+        ref = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, nx, ny)
+        assert _err(_gpu_map(torch, lt, W, lt.LT_FP64, nx=nx, ny=ny), ref) < TOL_F64
+        m = _gpu_map(torch, lt, W, lt.LT_MIXED, nx=nx, ny=ny)
+        assert np.abs(m - ref).max() / np.abs(ref).max() < TOL_F32
+    # pixel exactly on a lens centre, circular lens (e = 0), more lenses than one chunk
+    L = workloads.random_catalogue(77, 700, L=20.0)
+    L[0, 2] = 0.0
+    L[1, 2] = 0.0
+    L[1, 0], L[1, 1] = 0.0, 0.0
+    W2 = workloads.Workload("edge", L, -8.0, -8.0, 0.5, 40, 36, 77)      # pixel (16,16) = (0,0) = centre of lens 1
+    ref = O.gradient_grid(W2.lenses, W2.x_min, W2.y_min, W2.dx, W2.nx, W2.ny)
+    assert _err(_gpu_map(torch, lt, W2, lt.LT_FP64), ref) < TOL_F64
+    assert _err(_gpu_map(torch, lt, W2, lt.LT_FP32), ref) < TOL_F32
+    one = workloads.Workload("centre", L[1:2], 0.0, 0.0, 0.5, 1, 1, 0)
+    assert np.all(_gpu_map(torch, lt, one, lt.LT_FP64) == 0)
+
+
+def test_error_codes_and_bad_lens(env):
+    torch, lt, O = env
+    W = workloads.make(0)
+    L = torch.from_numpy(W.lenses).cuda()
+    with pytest.raises(lt.LtError) as e:
+        lt.lt_gradient_grid(L, 0.0, 0.0, -1.0, 8, 8)
+    assert e.value.code == -3
+    with pytest.raises(lt.LtError) as e:
+        lt.lt_gradient_grid(L, 0.0, 0.0, 1.0, 8, 8, mode=7, out=torch.empty((8, 8, 2), dtype=torch.float64, device="cuda"),
+                            workspace=torch.empty(1 << 16, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == -4
+    with pytest.raises(lt.LtError) as e:
+        lt.lt_gradient_grid(L, 0.0, 0.0, 1.0, 8, 8, workspace=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == -5
+    bad = W.lenses.copy()
+    bad[3, 5] = bad[3, 4] * 0.5           # rcut < rcore
+    ws = lt.alloc_workspace(len(bad), 8, 8, lt.LT_FP64)
+    out = lt.lt_gradient_grid(torch.from_numpy(bad).cuda(), 0.0, 0.0, 1.0, 8, 8, workspace=ws)
+    rc, k = lt.lt_last_status(ws)
+    assert rc == lt.LT_ERR_BAD_LENS_PARAMS and k == 3
+    assert torch.isnan(out).all()
+
+
+def test_host_buffer_entry_point(env):
+    torch, lt, O = env
+    W = workloads.make(0)
+    hL = torch.from_numpy(W.lenses).pin_memory()
+    for mode, dt in ((lt.LT_FP64, torch.float64), (lt.LT_FP32, torch.float32), (lt.LT_MIXED, torch.float64)):
+        hout = torch.empty((W.ny, W.nx, 2), dtype=dt).pin_memory()
+        ws = lt.alloc_workspace(len(W.lenses), W.nx, W.ny, mode, host=True)
+        lt.lt_gradient_grid_host(hL, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, hout, ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(hout.numpy(), _gpu_map(torch, lt, W, mode))
