@@ -1,0 +1,382 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the deflection-map hot path on synthetic cluster catalogues.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--mode fp64|fp32|mixed] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch: one lt_gradient_grid call (per-lens precompute kernel +
+gradient kernel [+ patch / flag / compaction kernels + fp64 recompute for mixed]) on BASELINE.json config 1
+(1024 x 1024 pixels over [-100,100]", 1 cluster-scale + 99 galaxy-scale dPIE halos, seed 1001; recipe in DESIGN.md
+section 4).  The headline `value` is the fp64 mode (the paper's DP run, Table 2); the same line carries
+the fp32 and mixed numbers on the same workload under "modes".
+
+Timing: CUDA events on the launching stream around every step, W >= 3 warm-up steps, L2 flushed (a 256 MiB buffer
+is overwritten) between timed steps outside the event pairs, barrier + torch.cuda.synchronize() on both sides of the
+timed region, max over ranks.  `value` has the catalogue already resident in HBM; `e2e` goes through
+lt_gradient_grid_host with pinned HOST buffers (H2D of the catalogue and D2H of the whole map inside the timed region).
+
+N > 1 (torchrun, one rank per GPU): the path shards with no exchange (pixels and MCMC samples are independent,
+P:98): every rank computes the full map of its OWN catalogue (seed + rank) -- weak scaling, no collective
+on the data path; NCCL is used only for the barrier and the max over ranks.
+
+--impl reference: times the CPU oracle (oracle/lt_oracle.cpp, `double` instantiation, as it stands) on the host cores,
+each step a bounded row sample of the same workload; rank 0 only.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "lens_pixel_gradient_evals_per_s"
+UNIT = "lens*pixel/s"
+MODES = {"fp64": 0, "fp32": 1, "mixed": 2}
+DTYPE = {"fp64": "f64", "fp32": "f32", "mixed": "f32+f64"}
+
+# FLOP-count convention per lens-pixel interaction (DESIGN.md section 8 / SURVEY 8(d)): textbook evaluation with
+# per-lens constants precomputed, add/sub/mul = 1, FMA = 2: 61 flops + 8 specials (2 sqrt, 2 div, 2 ln, 2 atan2).
+F_NOM = 69.0
+# lanes per SM behind the "alu" peaks (paper's Table 1 convention: 2 ops/cycle x clock x lanes)
+LANES = {"fp64": 64, "fp32": 128, "mixed": 64}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at config 1, from the ncu --set full
+# capture summarised in profiles/ (r01_*); None until captured.
+NCU_TRAFFIC_BYTES = {"fp64": None, "fp32": None, "mixed": None}
+KERNEL_NAME = {"fp64": "lt_grad_f64_kernel", "fp32": "lt_grad_f32_kernel", "mixed": "lt_grad_list_f64_kernel"}
+# kernels of ours launched per step (cudaMemsetAsync nodes are not counted)
+LAUNCHES_PER_STEP = {"fp64": 2, "fp32": 2, "mixed": 5}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = the metric's)")
+    ap.add_argument("--mode", default="fp64", choices=list(MODES))
+    ap.add_argument("--paper-regime", action="store_true", help="light galaxy halos (DESIGN.md section 4)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the other modes, cpu_baseline and peak probes")
+    ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU work of the oracle sample")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------ helpers
+class ClockSampler:
+    """Samples SM clock and clock-event reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.02):
+        self.samples, self.reasons, self.power = [], set(), []
+        self.period, self.ok, self._stop = period, False, threading.Event()
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            self.nv, self.h = nv, nv.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # noqa: BLE001 -- NVML missing is reported, not fatal
+            self.err = repr(e)
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksEventReasonHwPowerBrakeSlowdown: "hw_power_brake",
+                 nv.nvmlClocksEventReasonApplicationsClocksSetting: "applications_clocks_setting"}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.ok:
+            self.t.start()
+
+    def stop(self):
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
+        self._stop.set()
+        self.t.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+def physical_index(local):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local])
+        except (ValueError, IndexError):
+            return local
+    return local
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:  # noqa: BLE001
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def oracle_sample(W, cpu_seconds, ns_per_interaction=350.0):
+    """Row stride so that the `double` oracle does about `cpu_seconds` of CPU work on this workload."""
+    total = W.nx * W.ny * len(W.lenses) * ns_per_interaction * 1e-9
+    stride = max(1, int(round(total / cpu_seconds)))
+    rows = (W.ny + stride - 1) // stride
+    return stride, rows
+
+
+def time_oracle(W, stride, threads=0):
+    from oracle import lt_oracle as O
+    O.lib()
+    t0 = time.perf_counter()
+    O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, precision=O.DOUBLE, n_threads=threads,
+                    row_stride=stride)
+    dt = time.perf_counter() - t0
+    rows = (W.ny + stride - 1) // stride
+    return rows * W.nx * len(W.lenses) / dt, dt
+
+
+def run_reference(args, W):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import lt_oracle as O
+    cores = O.max_threads()
+    # every step = one bounded sample; the whole run (warmup + steps) is sized to stay within ~2 minutes of wall time
+    budget = 100.0 * cores / max(1, args.steps + args.warmup)
+    stride, rows = oracle_sample(W, min(args.cpu_seconds, budget))
+    for _ in range(args.warmup):
+        time_oracle(W, stride)
+    t = []
+    for _ in range(args.steps):
+        v, dt = time_oracle(W, stride)
+        t.append(dt)
+    ms = 1e3 * sum(t) / len(t)
+    units = rows * W.nx * len(W.lenses)
+    value = units / (ms * 1e-3)
+    sample = "rows 0,%d,2*%d,... (%d of %d rows) of %s, all pixels of each row, `double` instantiation" % (
+        stride, stride, rows, W.ny, W.name)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": W.name, "n_lens": int(len(W.lenses)), "nx": W.nx, "ny": W.ny, "seed": W.seed,
+                       "mode": "fp64", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+class Runner:
+    """Holds the device buffers of one workload/mode and issues steps through the C ABI (python = marshalling)."""
+
+    def __init__(self, torch, lt, W, mode):
+        self.torch, self.lt, self.W, self.mode = torch, lt, W, mode
+        self.code = MODES[mode]
+        n = len(W.lenses)
+        self.d_lenses = torch.from_numpy(W.lenses).cuda()
+        dt = torch.float32 if mode == "fp32" else torch.float64
+        self.out = torch.empty((W.ny, W.nx, 2), dtype=dt, device="cuda")
+        self.ws = lt.alloc_workspace(n, W.nx, W.ny, self.code)
+        self.h_lenses = torch.from_numpy(W.lenses).pin_memory()
+        self.h_out = torch.empty((W.ny, W.nx, 2), dtype=dt).pin_memory()
+        self.ws_host = lt.alloc_workspace(n, W.nx, W.ny, self.code, host=True)
+        self.units = W.nx * W.ny * n
+        self.h2d = self.h_lenses.numel() * 8
+        self.d2h = self.h_out.numel() * self.h_out.element_size()
+
+    def step(self):
+        W = self.W
+        self.lt.lt_gradient_grid(self.d_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, out=self.out,
+                                 workspace=self.ws)
+
+    def step_host(self):
+        W = self.W
+        self.lt.lt_gradient_grid_host(self.h_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, self.h_out,
+                                      self.ws_host)
+
+
+def timed(torch, lt, fn, steps, warmup, flush, barrier):
+    """W warm-up steps, then K steps each bracketed by CUDA events on the current stream; L2 flushed between steps
+    (outside the event pairs).  A second event pair per step, recorded by the library itself around the dominant
+    kernel's launch (lt_set_kernel_events), gives that kernel's duration inside the same timed region.
+    Returns (mean step time [ms], mean dominant-kernel time [ms])."""
+    for _ in range(warmup):
+        fn()
+        flush.fill_(1)
+
+    def pairs():
+        out = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in out:          # force the lazy cudaEventCreate before the timed region
+            a.record()
+            b.record()
+        return out
+    ev, kev = pairs(), pairs()
+    torch.cuda.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    for (a, b), (ka, kb) in zip(ev, kev):
+        lt.lt_set_kernel_events(ka, kb)
+        a.record()
+        fn()
+        b.record()
+        flush.fill_(1)
+    torch.cuda.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    lt.lt_set_kernel_events(None, None)
+    return sum(a.elapsed_time(b) for a, b in ev) / steps, sum(a.elapsed_time(b) for a, b in kev) / steps
+
+
+def run_ours(args, W):
+    import torch
+    from paper_1902_03252_b200 import lt
+    lt.lib()                                          # raises if the CUDA library is missing: no fallback
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference)")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        from paper_1902_03252_b200 import workloads
+        W = workloads.make(args.config, paper_regime=args.paper_regime, seed_offset=rank)   # own catalogue per rank
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    peaks, peak_src = measured_peaks()
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    sampler = ClockSampler(physical_index(local))
+
+    def measure(mode, steps, warmup, host=False):
+        r = Runner(torch, lt, W, mode)
+        fn = r.step_host if host else r.step
+        ms, ms_kernel = timed(torch, lt, fn, steps, warmup, flush, barrier)
+        rc, bad = lt.lt_last_status(r.ws_host if host else r.ws)
+        if rc != 0:
+            raise RuntimeError("lens parameter domain error at lens %d" % bad)
+        r.ms_kernel = ms_kernel
+        if dist is not None:
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        extra = {}
+        if mode == "mixed":
+            st = lt.lt_mixed_last_stats(r.ws_host if host else r.ws)
+            extra = {"flagged_fraction": st["n_flagged"] / (W.nx * W.ny), "patch_fraction": st["n_patch"] / (W.nx * W.ny),
+                     "eq25_fraction": st["n_eq25"] / (W.nx * W.ny), "eq28_fraction": st["n_eq28"] / (W.nx * W.ny)}
+        return r, ms, extra
+
+    # ---- headline: the requested mode, device-resident inputs
+    sampler.start()
+    r, ms, extra = measure(args.mode, args.steps, args.warmup)
+    value = world * r.units / (ms * 1e-3)
+    # ---- e2e: same metric through the host-buffer entry point
+    e2e_steps = max(3, min(args.steps, 50))
+    _, ms_e2e, _ = measure(args.mode, e2e_steps, max(3, min(args.warmup, 5)), host=True)
+    clocks = sampler.stop()
+
+    ms_kernel_main = r.ms_kernel        # dominant kernel, events recorded by the library inside the timed steps
+    sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0)
+
+    def roofline(mode, ms_k, units, flagged=1.0):
+        # mixed: the dominant kernel is the fp64 recompute, which processes the flagged pixels only
+        units = units * flagged
+        peak = 2.0 * sms * LANES[mode] * sm_max * 1e6 / 1e12
+        ach = F_NOM * units / (ms_k * 1e-3) / 1e12
+        return {"bound": "alu", "kernel": KERNEL_NAME[mode], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES[mode],
+                "peak_source": "derived: 2 x %d SMs x %d lanes x %.0f MHz (DESIGN.md section 8); no FP%s vector peak in "
+                               "MEASURED_PEAKS.json (%s)" % (sms, LANES[mode], sm_max, "64" if LANES[mode] == 64 else "32",
+                                                             peak_src),
+                "flops_per_interaction_nominal": F_NOM, "duration_ms": ms_k,
+                "interactions_per_launch": units,
+                "algorithmic_bytes_per_launch": r.out.numel() * r.out.element_size()}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": DTYPE[args.mode], "data": "synthetic",
+            "config": {"workload": W.name, "n_lens": int(len(W.lenses)), "nx": W.nx, "ny": W.ny, "seed": W.seed,
+                       "mode": args.mode, "parallelism": "dp%d (independent catalogues, no exchange)" % world,
+                       "l2": "256 MiB buffer overwritten between timed steps", "inputs": "resident in HBM"},
+            "clocks": clocks,
+            "e2e": {"value": world * r.units / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": r.h2d, "d2h_bytes_per_step": r.d2h,
+                    "api": "lt_gradient_grid_host (pinned host catalogue in, pinned host map out)"},
+            "gpu_launches": LAUNCHES_PER_STEP[args.mode] * args.steps,
+            "roofline": roofline(args.mode, ms_kernel_main, r.units, extra.get("flagged_fraction", 1.0))}
+    line.update(extra)
+
+    if not args.no_extras:
+        modes = {args.mode: {"value": value, "ms_per_step": ms, **extra}}
+        for m in MODES:
+            if m == args.mode:
+                continue
+            rm, ms_m, ex = measure(m, max(3, min(args.steps, 50)), max(3, min(args.warmup, 5)))
+            modes[m] = {"value": world * rm.units / (ms_m * 1e-3), "ms_per_step": ms_m, **ex,
+                        "kernel_ms": rm.ms_kernel,
+                        "roofline_frac_nominal": roofline(m, rm.ms_kernel, rm.units,
+                                                          ex.get("flagged_fraction", 1.0))["frac"]}
+        line["modes"] = modes
+        if rank == 0:
+            p64, p32 = lt.lt_peak_probe(0, 1 << 15), lt.lt_peak_probe(1, 1 << 16)
+            line["peak_probe"] = {"fp64_tflops": p64 / 1e12, "fp32_tflops": p32 / 1e12,
+                                  "how": "dependent-free FMA chains, full grid, same process"}
+            line["roofline"]["frac_of_probe"] = line["roofline"]["achieved"] / (
+                (p64 if LANES[args.mode] == 64 else p32) / 1e12)
+        if rank == 0 and world == 1:
+            from oracle import lt_oracle as O   # the cpu_baseline leg: the one place bench.py runs the oracle
+            stride, rows = oracle_sample(W, args.cpu_seconds)
+            v, dt = time_oracle(W, stride)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
+                                    "seconds": dt,
+                                    "sample": "rows 0,%d,... (%d of %d rows) of %s, `double` instantiation, "
+                                              "OpenMP over rows" % (stride, rows, W.ny, W.name)}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    from paper_1902_03252_b200 import workloads
+    W = workloads.make(args.config, paper_regime=args.paper_regime)
+    if args.impl == "reference":
+        run_reference(args, W)
+    else:
+        run_ours(args, W)
+
+
+if __name__ == "__main__":
+    main()

@@ -130,6 +130,14 @@ int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens,
  */
 int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm);
 
+/*
+ * Measurement hook for bench.py's roofline figure: two cudaEvent_t (as void*; both NULL switches the hook off) that the
+ * NEXT calls of lt_gradient_grid on this host thread record on cuda_stream immediately before and after the launch of
+ * the dominant kernel (fp64 / fp32 grid kernel; for LT_MIXED the fp64 recompute kernel), so that its duration can be
+ * taken on the launching stream without a profiler.  Returns LT_ERR_NULL_POINTER if exactly one is NULL.
+ */
+int lt_set_kernel_events(void* ev_start, void* ev_stop);
+
 /* After a call on this workspace: LT_OK or LT_ERR_BAD_LENS_PARAMS (first offending lens index in *bad_lens_or_null).
  * Synchronises cuda_stream. */
 int lt_last_status(const void* d_workspace, void* cuda_stream, int* bad_lens_or_null);

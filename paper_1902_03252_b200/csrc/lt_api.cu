@@ -19,6 +19,7 @@ struct Tuning {
   int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0;
 };
 Tuning g_tuning;
+thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
 
 constexpr int kDefaultChunk64 = 256;   // 32 KB of fp64 records per CTA
 constexpr int kDefaultChunk32 = 1024;  // 64 KB of fp32 records per CTA
@@ -114,6 +115,18 @@ int pick_ppt(int wanted, int max_ppt, int nx, int ny, const DeviceInfo& d) {
   return ppt;
 }
 
+// records the measurement-hook events around the dominant kernel's launch
+struct KernelEvents {
+  cudaStream_t st;
+  bool on;
+  explicit KernelEvents(cudaStream_t s, bool enable = true) : st(s), on(enable && g_ev_start && g_ev_stop) {
+    if (on) cudaEventRecord(g_ev_start, st);
+  }
+  ~KernelEvents() {
+    if (on) cudaEventRecord(g_ev_stop, st);
+  }
+};
+
 struct GridArgs {
   int n_lens;
   double x_min, y_min, dx;
@@ -130,6 +143,7 @@ int launch_f64_ppt(const LtLens<double>* l64, const GridArgs& a, double2* out, c
   int grid = 1;
   const int rc = grid_for(lt_grad_f64_kernel<PPT>, smem, n_tiles, d, grid);
   if (rc != LT_OK) return rc;
+  KernelEvents ke(st);
   lt_grad_f64_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny,
                                                          tiles_x, (int)n_tiles, out);
   LT_CUDA(cudaGetLastError());
@@ -144,7 +158,7 @@ int launch_f64(const LtLens<double>* l64, const GridArgs& a, double2* out, const
 
 template <int PPT>
 int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const GridArgs& a, float2* out,
-                   const DeviceInfo& d, cudaStream_t st) {
+                   const DeviceInfo& d, cudaStream_t st, bool hook) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
                                sizeof(LtLens<float>), d);
   const size_t smem = (size_t)chunk * sizeof(LtLens<float>);
@@ -153,17 +167,18 @@ int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const Gr
   int grid = 1;
   const int rc = grid_for(lt_grad_f32_kernel<PPT>, smem, n_tiles, d, grid);
   if (rc != LT_OK) return rc;
+  KernelEvents ke(st, hook);
   lt_grad_f32_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, l32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
                                                          a.ny, tiles_x, (int)n_tiles, out);
   LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
 int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const GridArgs& a, float2* out,
-               const DeviceInfo& d, cudaStream_t st) {
+               const DeviceInfo& d, cudaStream_t st, bool hook = true) {
   switch (pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d)) {
-    case 1: return launch_f32_ppt<1>(l64, l32, a, out, d, st);
-    case 2: return launch_f32_ppt<2>(l64, l32, a, out, d, st);
-    default: return launch_f32_ppt<4>(l64, l32, a, out, d, st);
+    case 1: return launch_f32_ppt<1>(l64, l32, a, out, d, st, hook);
+    case 2: return launch_f32_ppt<2>(l64, l32, a, out, d, st, hook);
+    default: return launch_f32_ppt<4>(l64, l32, a, out, d, st, hook);
   }
 }
 
@@ -177,6 +192,7 @@ int launch_list(const LtLens<double>* l64, const GridArgs& a, const unsigned int
   int grid = 1;
   const int rc = grid_for(lt_grad_list_f64_kernel<FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
   if (rc != LT_OK) return rc;
+  KernelEvents ke(st, FROM_LIST);
   lt_grad_list_f64_kernel<FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
                                                                     a.nx, list, hdr, points, n_points, out);
   LT_CUDA(cudaGetLastError());
@@ -267,6 +283,13 @@ int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_s
   return LT_OK;
 }
 
+int lt_set_kernel_events(void* ev_start, void* ev_stop) {
+  if ((ev_start == nullptr) != (ev_stop == nullptr)) return LT_ERR_NULL_POINTER;
+  g_ev_start = (cudaEvent_t)ev_start;
+  g_ev_stop = (cudaEvent_t)ev_stop;
+  return LT_OK;
+}
+
 size_t lt_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode) {
   if (!sizes_ok(n_lens, nx, ny)) return 0;
   if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return 0;
@@ -323,7 +346,7 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y
                                             nx, ny, md, flags);
     LT_CUDA(cudaGetLastError());
   }
-  rc = launch_f32(l64, l32, a, sp, dev, st);
+  rc = launch_f32(l64, l32, a, sp, dev, st, /*hook=*/false);
   if (rc != LT_OK) return rc;
   {
     long long blocks = (n_pix + 255) / 256;

@@ -21,7 +21,7 @@ _LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
 
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
-           "lt_set_tuning", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
+           "lt_set_tuning", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
 
 
 class lt_mixed_params(ctypes.Structure):
@@ -73,6 +73,8 @@ def lib():
         L.lt_gradient_points.restype = ci
         L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci]
         L.lt_set_tuning.restype = ci
+        L.lt_set_kernel_events.argtypes = [vp, vp]
+        L.lt_set_kernel_events.restype = ci
         L.lt_last_status.argtypes = [vp, vp, ctypes.POINTER(ci)]
         L.lt_last_status.restype = ci
         L.lt_mixed_last_stats.argtypes = [vp, vp, ctypes.POINTER(lt_mixed_stats)]
@@ -132,6 +134,18 @@ def lt_host_workspace_bytes(n_lens, nx, ny, mode):
 
 def lt_set_tuning(ppt64=0, ppt32=0, chunk64=0, chunk32=0, ctas_per_sm=0):
     _check(lib().lt_set_tuning(int(ppt64), int(ppt32), int(chunk64), int(chunk32), int(ctas_per_sm)), "lt_set_tuning")
+
+
+def lt_set_kernel_events(ev_start=None, ev_stop=None):
+    """Measurement hook: two torch.cuda.Event(enable_timing=True) recorded by the next lt_gradient_grid calls around
+    the dominant kernel's launch; None, None switches it off."""
+    def handle(ev):
+        if ev is None:
+            return None
+        if not ev.cuda_event:       # torch creates the cudaEvent lazily: force it
+            ev.record()
+        return ctypes.c_void_p(ev.cuda_event)
+    _check(lib().lt_set_kernel_events(handle(ev_start), handle(ev_stop)), "lt_set_kernel_events")
 
 
 def alloc_workspace(n_lens, nx, ny, mode, device="cuda", host=False):

@@ -43,14 +43,16 @@ def _cluster(rng):
                      rng.uniform(5.0, 20.0), rng.uniform(500.0, 1000.0), rng.uniform(20.0, 30.0)])
 
 
-def make(cfg, paper_regime=False, n_override=None):
+def make(cfg, paper_regime=False, n_override=None, seed_offset=0):
     """Workload for BASELINE.json config `cfg` (0..4).
 
     paper_regime: galaxy-scale b0 x 0.05 and rcut x 0.3 (cluster halo unchanged) -- the lens-physically light variant
     on which the mixed rule flags a few percent of the pixels as in the paper's Fig. 7.
     n_override: use an n x n grid over the same extent instead (parity tests at reduced size).
+    seed_offset: added to the config's seed (bench.py --gpus N: rank r draws its own catalogue with seed + r).
     """
     name, n, L, n_lens, seed = _CONFIGS[cfg]
+    seed += int(seed_offset)
     rng = np.random.default_rng(seed)
     if n_override is not None:
         n = int(n_override)
