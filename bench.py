@@ -137,7 +137,7 @@ def measured_peaks():
 
 
 # ------------------------------------------------------------------------------------------------ reference arm
-def oracle_sample(W, cpu_seconds, ns_per_interaction=350.0):
+def oracle_sample(W, cpu_seconds, ns_per_interaction=100.0):
     """Row stride so that the `double` oracle does about `cpu_seconds` of CPU work on this workload."""
     total = W.nx * W.ny * len(W.lenses) * ns_per_interaction * 1e-9
     stride = max(1, int(round(total / cpu_seconds)))
