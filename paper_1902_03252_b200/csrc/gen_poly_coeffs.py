@@ -66,14 +66,14 @@ def emit(name, g, zmax, n, rnd, suffix):
 
 
 if __name__ == "__main__":
-    import sys
-    zt = mp.tan(mp.pi / 8) * (1 + mp.mpf(10) ** -5)          # 3-way atan reduction leaves |z| <= tan(pi/8)
-    zh = mp.mpf('0.21')     # bit-pattern log2 reduction: |log2 ratio| <= 0.5 + 0.087 -> |z| <= 0.2004
-    for n in (10, 11, 12, 13):
-        emit("LT_ATAN_P64_%d" % n, g_atan, zt, n, float, "")
-    for n in (6, 7, 8, 9):
-        emit("LT_ATANH_P64_%d" % n, g_atanh, zh, n, float, "")
-    for n in (3, 4, 5, 6):
-        emit("LT_ATAN_P32_%d" % n, g_atan, zt, n, f32, "f")
-    for n in (2, 3, 4):
-        emit("LT_ATANH_P32_%d" % n, g_atanh, zh, n, f32, "f")
+    # table-driven range reductions of lt_math.cuh (quarter-octave bins chosen from the operands' bit patterns) leave
+    # |z| <= 0.0702 (atan, rotation table) and |z| <= 0.0724 (atanh, scale table); fitted on |z| <= 0.075
+    zr = mp.mpf('0.075')
+    for n in (4, 5, 6):
+        emit("LT_ATAN_P64_%d" % n, g_atan, zr, n, float, "")
+    for n in (4, 5, 6):
+        emit("LT_ATANH_P64_%d" % n, g_atanh, zr, n, float, "")
+    for n in (1, 2, 3):
+        emit("LT_ATAN_P32_%d" % n, g_atan, zr, n, f32, "f")
+    for n in (1, 2, 3):
+        emit("LT_ATANH_P32_%d" % n, g_atanh, zr, n, f32, "f")

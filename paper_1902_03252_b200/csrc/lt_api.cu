@@ -28,13 +28,15 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t header, lens64, lens32, flags, sp, list, total;
+  size_t header, tab64, tab32, lens64, lens32, flags, sp, list, total;
 };
 
 Layout make_layout(int n_lens, long long n_pix, bool mixed) {
   Layout L;
   size_t o = 0;
   L.header = o; o += sizeof(LtWsHeader);
+  L.tab64 = o;  o += align_up(sizeof(LtTables<double>));
+  L.tab32 = o;  o += align_up(sizeof(LtTables<float>));
   L.lens64 = o; o += align_up((size_t)n_lens * sizeof(LtLens<double>));
   L.lens32 = o; o += align_up((size_t)n_lens * sizeof(LtLens<float>));
   L.flags = o;  if (mixed) o += align_up((size_t)n_pix);
@@ -96,7 +98,7 @@ int grid_for(K kernel, size_t smem, long long n_work, const DeviceInfo& d, int& 
 
 int pick_chunk(int n_lens, int wanted, size_t rec_bytes, const DeviceInfo& d) {
   int chunk = wanted;
-  const int max_chunk = (int)((d.smem_optin - 1024) / rec_bytes);
+  const int max_chunk = (int)((d.smem_optin - 4096) / rec_bytes   /* static smem: the range-reduction tables */);
   if (chunk > max_chunk) chunk = max_chunk;
   if (chunk > n_lens) chunk = n_lens;
   if (chunk < 1) chunk = 1;
@@ -134,7 +136,7 @@ struct GridArgs {
 };
 
 template <int PPT>
-int launch_f64_ppt(const LtLens<double>* l64, const GridArgs& a, double2* out, const DeviceInfo& d, cudaStream_t st) {
+int launch_f64_ppt(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out, const DeviceInfo& d, cudaStream_t st) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
                                sizeof(LtLens<double>), d);
   const size_t smem = (size_t)chunk * sizeof(LtLens<double>);
@@ -144,20 +146,22 @@ int launch_f64_ppt(const LtLens<double>* l64, const GridArgs& a, double2* out, c
   const int rc = grid_for(lt_grad_f64_kernel<PPT>, smem, n_tiles, d, grid);
   if (rc != LT_OK) return rc;
   KernelEvents ke(st);
-  lt_grad_f64_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny,
+  lt_grad_f64_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny,
                                                          tiles_x, (int)n_tiles, out);
   LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
-int launch_f64(const LtLens<double>* l64, const GridArgs& a, double2* out, const DeviceInfo& d, cudaStream_t st) {
+int launch_f64(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
+               const DeviceInfo& d, cudaStream_t st) {
   switch (pick_ppt(g_tuning.ppt64, 2, a.nx, a.ny, d)) {
-    case 1: return launch_f64_ppt<1>(l64, a, out, d, st);
-    default: return launch_f64_ppt<2>(l64, a, out, d, st);
+    case 1: return launch_f64_ppt<1>(l64, t64, a, out, d, st);
+    default: return launch_f64_ppt<2>(l64, t64, a, out, d, st);
   }
 }
 
 template <int PPT>
-int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const GridArgs& a, float2* out,
+int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32,
+                   const GridArgs& a, float2* out,
                    const DeviceInfo& d, cudaStream_t st, bool hook) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
                                sizeof(LtLens<float>), d);
@@ -168,22 +172,22 @@ int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const Gr
   const int rc = grid_for(lt_grad_f32_kernel<PPT>, smem, n_tiles, d, grid);
   if (rc != LT_OK) return rc;
   KernelEvents ke(st, hook);
-  lt_grad_f32_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, l32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
+  lt_grad_f32_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
                                                          a.ny, tiles_x, (int)n_tiles, out);
   LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
-int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const GridArgs& a, float2* out,
-               const DeviceInfo& d, cudaStream_t st, bool hook = true) {
+int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32, const GridArgs& a,
+               float2* out, const DeviceInfo& d, cudaStream_t st, bool hook = true) {
   switch (pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d)) {
-    case 1: return launch_f32_ppt<1>(l64, l32, a, out, d, st, hook);
-    case 2: return launch_f32_ppt<2>(l64, l32, a, out, d, st, hook);
-    default: return launch_f32_ppt<4>(l64, l32, a, out, d, st, hook);
+    case 1: return launch_f32_ppt<1>(l64, l32, t32, a, out, d, st, hook);
+    case 2: return launch_f32_ppt<2>(l64, l32, t32, a, out, d, st, hook);
+    default: return launch_f32_ppt<4>(l64, l32, t32, a, out, d, st, hook);
   }
 }
 
 template <bool FROM_LIST>
-int launch_list(const LtLens<double>* l64, const GridArgs& a, const unsigned int* list, const LtWsHeader* hdr,
+int launch_list(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, const unsigned int* list, const LtWsHeader* hdr,
                 const double2* points, long long n_points, long long max_work, double2* out, const DeviceInfo& d,
                 cudaStream_t st) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
@@ -193,7 +197,7 @@ int launch_list(const LtLens<double>* l64, const GridArgs& a, const unsigned int
   const int rc = grid_for(lt_grad_list_f64_kernel<FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
   if (rc != LT_OK) return rc;
   KernelEvents ke(st, FROM_LIST);
-  lt_grad_list_f64_kernel<FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
+  lt_grad_list_f64_kernel<FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
                                                                     a.nx, list, hdr, points, n_points, out);
   LT_CUDA(cudaGetLastError());
   return LT_OK;
@@ -213,6 +217,8 @@ int precompute(const lt_lens* d_lenses, int n_lens, double dx, unsigned char* ws
   lt_precompute_kernel<<<blocks, 128, 0, st>>>(reinterpret_cast<const LtRawLens*>(d_lenses), n_lens, dx,
                                                reinterpret_cast<LtLens<double>*>(ws + L.lens64),
                                                reinterpret_cast<LtLens<float>*>(ws + L.lens32),
+                                               reinterpret_cast<LtTables<double>*>(ws + L.tab64),
+                                               reinterpret_cast<LtTables<float>*>(ws + L.tab32),
                                                reinterpret_cast<LtWsHeader*>(ws + L.header));
   LT_CUDA(cudaGetLastError());
   return LT_OK;
@@ -322,12 +328,14 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y
   LtWsHeader* hdr = reinterpret_cast<LtWsHeader*>(ws + L.header);
   const LtLens<double>* l64 = reinterpret_cast<const LtLens<double>*>(ws + L.lens64);
   const LtLens<float>* l32 = reinterpret_cast<const LtLens<float>*>(ws + L.lens32);
+  const LtTables<double>* t64 = reinterpret_cast<const LtTables<double>*>(ws + L.tab64);
+  const LtTables<float>* t32 = reinterpret_cast<const LtTables<float>*>(ws + L.tab32);
   const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
 
   rc = precompute(d_lenses, n_lens, dx, ws, L, st);                                   /* a1 */
   if (rc != LT_OK) return rc;
-  if (mode == LT_FP64) return launch_f64(l64, a, (double2*)d_out_grad, dev, st);      /* a2-a7 */
-  if (mode == LT_FP32) return launch_f32(l64, l32, a, (float2*)d_out_grad, dev, st);
+  if (mode == LT_FP64) return launch_f64(l64, t64, a, (double2*)d_out_grad, dev, st);      /* a2-a7 */
+  if (mode == LT_FP32) return launch_f32(l64, l32, t32, a, (float2*)d_out_grad, dev, st);
 
   /* LT_MIXED: single precision everywhere, flag, double precision on the flagged pixels */
   unsigned char* flags = ws + L.flags;
@@ -346,7 +354,7 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y
                                             nx, ny, md, flags);
     LT_CUDA(cudaGetLastError());
   }
-  rc = launch_f32(l64, l32, a, sp, dev, st, /*hook=*/false);
+  rc = launch_f32(l64, l32, t32, a, sp, dev, st, /*hook=*/false);
   if (rc != LT_OK) return rc;
   {
     long long blocks = (n_pix + 255) / 256;
@@ -355,7 +363,7 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y
     lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, (double2*)d_out_grad, list, hdr);   /* a8 */
     LT_CUDA(cudaGetLastError());
   }
-  return launch_list<true>(l64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
+  return launch_list<true>(l64, t64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
 }
 
 int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
@@ -373,7 +381,8 @@ int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_poin
   rc = precompute(d_lenses, n_lens, 1.0, ws, L, st);
   if (rc != LT_OK || n_points == 0) return rc;
   const GridArgs a{n_lens, 0.0, 0.0, 1.0, 1, 1};
-  return launch_list<false>(reinterpret_cast<const LtLens<double>*>(ws + L.lens64), a, nullptr,
+  return launch_list<false>(reinterpret_cast<const LtLens<double>*>(ws + L.lens64),
+                            reinterpret_cast<const LtTables<double>*>(ws + L.tab64), a, nullptr,
                             reinterpret_cast<const LtWsHeader*>(ws + L.header),
                             reinterpret_cast<const double2*>(d_points), n_points, n_points,
                             reinterpret_cast<double2*>(d_out), dev, st);

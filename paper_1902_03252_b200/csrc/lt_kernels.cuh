@@ -28,9 +28,12 @@ static_assert(sizeof(LtWsHeader) == 256, "workspace header is 256 bytes");
 // ------------------------------------------------------------------------------------------------ a1: precompute
 __global__ void lt_precompute_kernel(const LtRawLens* __restrict__ raw, int n_lens, double dx,
                                      LtLens<double>* __restrict__ l64, LtLens<float>* __restrict__ l32,
+                                     LtTables<double>* __restrict__ t64, LtTables<float>* __restrict__ t32,
                                      LtWsHeader* __restrict__ hdr) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k == 0) hdr->n_lens = n_lens;
+  if (blockIdx.x == gridDim.x - 1)           // the last block also writes the range-reduction tables (lt_math.cuh)
+    for (int e = threadIdx.x; e < LT_TABLE_ENTRIES; e += blockDim.x) lt_fill_table_entry(e, *t64, *t32);
   if (k >= n_lens) return;
   const LtRawLens r = raw[k];
   LtLens<double> D;
@@ -58,10 +61,14 @@ __device__ __forceinline__ void lt_copy16(void* dst, const void* src, int count)
 // lens (lt_interaction), a7 one double2 store per pixel.
 template <int PPT>
 __global__ void __launch_bounds__(LT_THREADS)
-lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, int n_lens, int chunk, double x_min, double y_min,
-                   double dx, int nx, int ny, int tiles_x, int n_tiles, double2* __restrict__ out) {
+lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<double>* __restrict__ tables, int n_lens,
+                   int chunk, double x_min, double y_min, double dx, int nx, int ny, int tiles_x, int n_tiles,
+                   double2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
+  __shared__ LtTables<double> tab;
   LtLens<double>* sl = reinterpret_cast<LtLens<double>*>(lt_smem);
+  lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  __syncthreads();
   constexpr int TILE_W = 32 * PPT;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   const bool single = n_lens <= chunk;
@@ -93,7 +100,7 @@ lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, int n_lens, int chun
         const LtLens<double> L = sl[k];
         const double d2 = t2 - L.y0;                                // Alg. 1 l.4
 #pragma unroll
-        for (int p = 0; p < PPT; ++p) lt_interaction<double>(t1[p] - L.x0, d2, L, G1[p], G2[p]);  // l.3, l.5-14
+        for (int p = 0; p < PPT; ++p) lt_interaction<double>(t1[p] - L.x0, d2, L, tab, G1[p], G2[p]);  // l.3, l.5-14
       }
     }
     if (j < ny) {
@@ -115,11 +122,13 @@ lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, int n_lens, int chun
 // (A.65)).  All per-interaction arithmetic is FP32.
 template <int PPT>
 __global__ void __launch_bounds__(LT_THREADS)
-lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float>* __restrict__ lens32, int n_lens,
-                   int chunk, double x_min, double y_min, double dx, int nx, int ny, int tiles_x, int n_tiles,
-                   float2* __restrict__ out) {
+lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float>* __restrict__ lens32,
+                   const LtTables<float>* __restrict__ tables, int n_lens, int chunk, double x_min, double y_min,
+                   double dx, int nx, int ny, int tiles_x, int n_tiles, float2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
+  __shared__ LtTables<float> tab;
   LtLens<float>* sl = reinterpret_cast<LtLens<float>*>(lt_smem);
+  lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));   // visible after the first __syncthreads of the chunk loop
   constexpr int TILE_W = 32 * PPT;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   // in-tile offsets from the tile centre, in pixels (exact in fp32)
@@ -161,10 +170,9 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
         for (int p = 0; p < PPT; ++p) {
           const float x = fmaf(il[p], L.dxc, xr);
           const float y = fmaf(-il[p], L.dxs, yr);
-          float gx, gy;
-          lt_dpie_body<float>(x, y, L, gx, gy);
-          G1[p] = fmaf(gx, L.c, fmaf(-gy, L.s, G1[p]));            // Alg. 1 l.10 + l.13
-          G2[p] = fmaf(gy, L.c, fmaf(gx, L.s, G2[p]));             // Alg. 1 l.11 + l.14
+          float ax, ay;
+          lt_dpie_body<float>(x, y, L, tab, ax, ay);
+          lt_accumulate<float>(ax, ay, L, G1[p], G2[p]);          // Alg. 1 l.10-11 + l.13-14
         }
       }
     }
@@ -184,11 +192,15 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
 // Uses the same lt_interaction in the same lens order as the fp64 grid kernel: identical bits for identical pixels.
 template <bool FROM_LIST>
 __global__ void __launch_bounds__(LT_THREADS)
-lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, int n_lens, int chunk, double x_min, double y_min,
-                        double dx, int nx, const unsigned int* __restrict__ list, const LtWsHeader* __restrict__ hdr,
+lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<double>* __restrict__ tables,
+                        int n_lens, int chunk, double x_min, double y_min, double dx, int nx,
+                        const unsigned int* __restrict__ list, const LtWsHeader* __restrict__ hdr,
                         const double2* __restrict__ points, long long n_points, double2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
+  __shared__ LtTables<double> tab;
   LtLens<double>* sl = reinterpret_cast<LtLens<double>*>(lt_smem);
+  lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  __syncthreads();
   const long long total = FROM_LIST ? (long long)hdr->list_count : n_points;
   const bool single = n_lens <= chunk;
   if (single) {
@@ -226,7 +238,7 @@ lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, int n_lens, int
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
         const LtLens<double> L = sl[k];
-        lt_interaction<double>(t1 - L.x0, t2 - L.y0, L, G1, G2);
+        lt_interaction<double>(t1 - L.x0, t2 - L.y0, L, tab, G1, G2);
       }
     }
     if (live) out[dst] = make_double2(G1, G2);

@@ -42,14 +42,14 @@ LT_HD void lt_pack_lens(const LtRawLens& r, double dx, LtLens<double>& L) {
   L.q2sc = q2 * sc;
   L.q2st = q2 * st;
   L.f = f;
-  L.C = r.b0 * (r.rcut / (r.rcut - r.rcore)) * ome / f;
-  L.pad = 0.0;
+  const double C = r.b0 * (r.rcut / (r.rcut - r.rcore)) * ome / f;
+  L.Cc = C * c;
+  L.Cs = C * s;
 }
 
 LT_HD void lt_poison_lens(LtLens<double>& L) {  // invalid parameters: the lens contributes NaN everywhere
   const double n = NAN;
-  L.x0 = L.y0 = L.c = L.s = L.dxc = L.dxs = L.q2 = L.Kc = L.Kt = L.sc = L.st = L.q2sc = L.q2st = L.f = L.C = n;
-  L.pad = 0.0;
+  L.x0 = L.y0 = L.c = L.s = L.dxc = L.dxs = L.q2 = L.Kc = L.Kt = L.sc = L.st = L.q2sc = L.q2st = L.f = L.Cc = L.Cs = n;
 }
 
 // fp32 record = fp64 record rounded once, except x0, y0 which the fp32 kernel fills per pixel tile (lens-frame
@@ -69,6 +69,6 @@ LT_HD void lt_round_lens(const LtLens<double>& D, LtLens<float>& F) {
   F.q2sc = (float)D.q2sc;
   F.q2st = (float)D.q2st;
   F.f = (float)D.f;
-  F.C = (float)D.C;
-  F.pad = 0.f;
+  F.Cc = (float)D.Cc;
+  F.Cs = (float)D.Cs;
 }
