@@ -124,7 +124,7 @@ int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens,
 
 /*
  * Launch-configuration knobs (process-wide; 0 = the library's default).  ppt64 / ppt32: pixels per thread of the
- * fp64 (1, 2) and fp32 (1, 2, 4) grid kernels; chunk64 / chunk32: lens records staged in shared memory at a time;
+ * fp64 (1, 2, 4) and fp32 (1, 2, 4) grid kernels; chunk64 / chunk32: lens records staged in shared memory at a time;
  * ctas_per_sm: cap on resident CTAs per SM of the persistent grids.  Results do not depend on any of them except
  * that the fp32 tile centre moves with ppt32.  Returns LT_ERR_BAD_SIZE on a negative value.
  */

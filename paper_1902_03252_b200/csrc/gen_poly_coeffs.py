@@ -66,12 +66,13 @@ def emit(name, g, zmax, n, rnd, suffix):
 
 
 if __name__ == "__main__":
-    # table-driven range reductions of lt_math.cuh (quarter-octave bins chosen from the operands' bit patterns) leave
-    # |z| <= 0.0702 (atan, rotation table) and |z| <= 0.0724 (atanh, scale table); fitted on |z| <= 0.075
-    zr = mp.mpf('0.075')
-    for n in (4, 5, 6):
+    # table-driven range reductions of lt_math.cuh (eighth-octave bins chosen from the operands' bit patterns: half a
+    # bin, 1/16 octave, plus the 0.0861 octave by which the piecewise-linear log2 of two bit patterns can be off) leave
+    # |z| <= (r - 1)/(r + 1), r = 2^0.1486, i.e. 0.0515 for both atan and atanh; fitted on |z| <= 0.053
+    zr = mp.mpf('0.053')
+    for n in (3, 4, 5):
         emit("LT_ATAN_P64_%d" % n, g_atan, zr, n, float, "")
-    for n in (4, 5, 6):
+    for n in (3, 4, 5):
         emit("LT_ATANH_P64_%d" % n, g_atanh, zr, n, float, "")
     for n in (1, 2, 3):
         emit("LT_ATAN_P32_%d" % n, g_atan, zr, n, f32, "f")

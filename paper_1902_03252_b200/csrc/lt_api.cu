@@ -135,7 +135,7 @@ struct GridArgs {
   int nx, ny;
 };
 
-template <int PPT>
+template <int PPT, int MINB>
 int launch_f64_ppt(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out, const DeviceInfo& d, cudaStream_t st) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
                                sizeof(LtLens<double>), d);
@@ -143,19 +143,22 @@ int launch_f64_ppt(const LtLens<double>* l64, const LtTables<double>* t64, const
   const int tiles_x = (a.nx + 32 * PPT - 1) / (32 * PPT), tiles_y = (a.ny + LT_TILE_H - 1) / LT_TILE_H;
   const long long n_tiles = (long long)tiles_x * tiles_y;
   int grid = 1;
-  const int rc = grid_for(lt_grad_f64_kernel<PPT>, smem, n_tiles, d, grid);
+  const int rc = grid_for(lt_grad_f64_kernel<PPT, MINB>, smem, n_tiles, d, grid);
   if (rc != LT_OK) return rc;
   KernelEvents ke(st);
-  lt_grad_f64_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny,
+  lt_grad_f64_kernel<PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny,
                                                          tiles_x, (int)n_tiles, out);
   LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
 int launch_f64(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
                const DeviceInfo& d, cudaStream_t st) {
-  switch (pick_ppt(g_tuning.ppt64, 2, a.nx, a.ny, d)) {
-    case 1: return launch_f64_ppt<1>(l64, t64, a, out, d, st);
-    default: return launch_f64_ppt<2>(l64, t64, a, out, d, st);
+  // 4 pixels per thread (4 independent chains, lens record loaded once per 4 interactions) at <= 128 registers, two
+  // CTAs per SM; fewer pixels per thread only for grids too small to give every SM two tiles
+  switch (pick_ppt(g_tuning.ppt64, 4, a.nx, a.ny, d)) {
+    case 1: return launch_f64_ppt<1, 4>(l64, t64, a, out, d, st);
+    case 2: return launch_f64_ppt<2, 3>(l64, t64, a, out, d, st);
+    default: return launch_f64_ppt<4, 2>(l64, t64, a, out, d, st);
   }
 }
 

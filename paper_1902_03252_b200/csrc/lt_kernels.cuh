@@ -38,13 +38,13 @@ __global__ void lt_precompute_kernel(const LtRawLens* __restrict__ raw, int n_le
   const LtRawLens r = raw[k];
   LtLens<double> D;
   if (lt_lens_valid(r)) {
-    lt_pack_lens(r, dx, D);
+    lt_pack_lens(r, D);
   } else {
     lt_poison_lens(D);
     atomicMax(&hdr->bad_code, n_lens - k);
   }
   LtLens<float> F;
-  lt_round_lens(D, F);
+  lt_round_lens(D, dx, F);
   l64[k] = D;
   l32[k] = F;
 }
@@ -59,8 +59,8 @@ __device__ __forceinline__ void lt_copy16(void* dst, const void* src, int count)
 // ------------------------------------------------------------------------------------------------ fp64 grid kernel
 // a2 pixel coordinate (x_min + i*dx, product and sum rounded separately, exactly as the API states it), a3-a6 per
 // lens (lt_interaction), a7 one double2 store per pixel.
-template <int PPT>
-__global__ void __launch_bounds__(LT_THREADS)
+template <int PPT, int MINB>
+__global__ void __launch_bounds__(LT_THREADS, MINB)
 lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<double>* __restrict__ tables, int n_lens,
                    int chunk, double x_min, double y_min, double dx, int nx, int ny, int tiles_x, int n_tiles,
                    double2* __restrict__ out) {
@@ -99,8 +99,9 @@ lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<doubl
       for (int k = 0; k < cnt; ++k) {
         const LtLens<double> L = sl[k];
         const double d2 = t2 - L.y0;                                // Alg. 1 l.4
+        const double d2sx = d2 * L.sx, d2cy = d2 * L.cy;
 #pragma unroll
-        for (int p = 0; p < PPT; ++p) lt_interaction<double>(t1[p] - L.x0, d2, L, tab, G1[p], G2[p]);  // l.3, l.5-14
+        for (int p = 0; p < PPT; ++p) lt_interaction<double>(t1[p] - L.x0, d2sx, d2cy, L, tab, G1[p], G2[p]);  // l.3, l.5-14
       }
     }
     if (j < ny) {
@@ -155,21 +156,21 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
       for (int k = threadIdx.x; k < cnt; k += LT_THREADS) {
         LtLens<float> F = lens32[base + k];
         const LtLens<double>& D = lens64[base + k];
-        const double d1 = cx - D.x0, d2 = cy - D.y0, c = D.c, s = D.s;
-        F.x0 = (float)fma(d1, c, d2 * s);
-        F.y0 = (float)fma(d2, c, -(d1 * s));
+        const double d1 = cx - D.x0, d2 = cy - D.y0;
+        F.x0 = (float)fma(d1, D.cx, d2 * D.sx);
+        F.y0 = (float)fma(-d1, D.sy, d2 * D.cy);
         sl[k] = F;
       }
       __syncthreads();
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
         const LtLens<float> L = sl[k];
-        const float xr = fmaf(jl, L.dxs, L.x0);
-        const float yr = fmaf(jl, L.dxc, L.y0);
+        const float xr = fmaf(jl, L.sx, L.x0);
+        const float yr = fmaf(jl, L.cy, L.y0);
 #pragma unroll
         for (int p = 0; p < PPT; ++p) {
-          const float x = fmaf(il[p], L.dxc, xr);
-          const float y = fmaf(-il[p], L.dxs, yr);
+          const float x = fmaf(il[p], L.cx, xr);
+          const float y = fmaf(-il[p], L.sy, yr);
           float ax, ay;
           lt_dpie_body<float>(x, y, L, tab, ax, ay);
           lt_accumulate<float>(ax, ay, L, G1[p], G2[p]);          // Alg. 1 l.10-11 + l.13-14
@@ -238,7 +239,8 @@ lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
         const LtLens<double> L = sl[k];
-        lt_interaction<double>(t1 - L.x0, t2 - L.y0, L, tab, G1, G2);
+        const double d2 = t2 - L.y0;
+        lt_interaction<double>(t1 - L.x0, d2 * L.sx, d2 * L.cy, L, tab, G1, G2);
       }
     }
     if (live) out[dst] = make_double2(G1, G2);

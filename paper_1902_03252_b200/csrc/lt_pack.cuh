@@ -18,7 +18,7 @@ LT_HD bool lt_lens_valid(const LtRawLens& r) {
 }
 
 // fp64 record.  x0, y0 = lens centre; dxc, dxs = dx cos Phi, dx sin Phi.
-LT_HD void lt_pack_lens(const LtRawLens& r, double dx, LtLens<double>& L) {
+LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
   double s, c;
   sincos(r.phi, &s, &c);
   const double e = r.e;
@@ -28,46 +28,47 @@ LT_HD void lt_pack_lens(const LtRawLens& r, double dx, LtLens<double>& L) {
   double f = 2.0 * sqrt(e) / ope;            // sqrt(1 - q^2)
   f = f < LT_F_MIN ? LT_F_MIN : f;           // e = 0 stays a regular point (header of lt_math.cuh)
   const double sc = r.rcore * ope, st = r.rcut * ope;
+  const double rf = 1.0 / f, qf = q * rf;
   L.x0 = r.x;
   L.y0 = r.y;
-  L.c = c;
-  L.s = s;
-  L.dxc = dx * c;
-  L.dxs = dx * s;
-  L.q2 = q2;
-  L.Kc = (ome * r.rcore) * (ome * r.rcore);  // q^2 s_c^2
-  L.Kt = (ome * r.rcut) * (ome * r.rcut);
-  L.sc = sc;
-  L.st = st;
-  L.q2sc = q2 * sc;
-  L.q2st = q2 * st;
+  L.cx = qf * c;
+  L.sx = qf * s;
+  L.cy = rf * c;
+  L.sy = rf * s;
+  L.Kc = (ome * r.rcore * rf) * (ome * r.rcore * rf);  // q^2 s_c^2 / f^2
+  L.Kt = (ome * r.rcut * rf) * (ome * r.rcut * rf);
+  L.sc = sc * rf;
+  L.st = st * rf;
+  L.q2sc = q2 * sc * rf;
+  L.q2st = q2 * st * rf;
+  L.g = f / q;
   L.f = f;
-  const double C = r.b0 * (r.rcut / (r.rcut - r.rcore)) * ome / f;
+  const double C = r.b0 * (r.rcut / (r.rcut - r.rcore)) * ome * rf;
   L.Cc = C * c;
   L.Cs = C * s;
 }
 
 LT_HD void lt_poison_lens(LtLens<double>& L) {  // invalid parameters: the lens contributes NaN everywhere
   const double n = NAN;
-  L.x0 = L.y0 = L.c = L.s = L.dxc = L.dxs = L.q2 = L.Kc = L.Kt = L.sc = L.st = L.q2sc = L.q2st = L.f = L.Cc = L.Cs = n;
+  L.x0 = L.y0 = L.cx = L.sx = L.cy = L.sy = L.Kc = L.Kt = L.sc = L.st = L.q2sc = L.q2st = L.g = L.f = L.Cc = L.Cs = n;
 }
 
 // fp32 record = fp64 record rounded once, except x0, y0 which the fp32 kernel fills per pixel tile (lens-frame
 // coordinates of the tile origin, formed in fp64 and then rounded: DESIGN.md section 5, "fp32 coordinates").
-LT_HD void lt_round_lens(const LtLens<double>& D, LtLens<float>& F) {
+LT_HD void lt_round_lens(const LtLens<double>& D, double dx, LtLens<float>& F) {
   F.x0 = 0.f;
   F.y0 = 0.f;
-  F.c = (float)D.c;
-  F.s = (float)D.s;
-  F.dxc = (float)D.dxc;
-  F.dxs = (float)D.dxs;
-  F.q2 = (float)D.q2;
+  F.cx = (float)(dx * D.cx);      // scaled lens-frame steps per pixel
+  F.sx = (float)(dx * D.sx);
+  F.cy = (float)(dx * D.cy);
+  F.sy = (float)(dx * D.sy);
   F.Kc = (float)D.Kc;
   F.Kt = (float)D.Kt;
   F.sc = (float)D.sc;
   F.st = (float)D.st;
   F.q2sc = (float)D.q2sc;
   F.q2st = (float)D.q2st;
+  F.g = (float)D.g;
   F.f = (float)D.f;
   F.Cc = (float)D.Cc;
   F.Cs = (float)D.Cs;
