@@ -125,10 +125,16 @@ int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens,
 /*
  * Launch-configuration knobs (process-wide; 0 = the library's default).  ppt64 / ppt32: pixels per thread of the
  * fp64 (1, 2, 4) and fp32 (1, 2, 4) grid kernels; chunk64 / chunk32: lens records staged in shared memory at a time;
- * ctas_per_sm: cap on resident CTAs per SM of the persistent grids.  Results do not depend on any of them except
- * that the fp32 tile centre moves with ppt32.  Returns LT_ERR_BAD_SIZE on a negative value.
+ * ctas_per_sm: cap on resident CTAs per SM of the persistent grids; single_launch: 1 = one launch of the chosen variant
+ * over the whole grid instead of whole waves plus a finer-grained rest.  Results do not depend on
+ * any of them except that the fp32 tile centre moves with the pixels per thread of the launch
+ * that owns the pixel.  Returns LT_ERR_BAD_SIZE on a negative value.
  */
-int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm);
+int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm, int single_launch);
+
+/* Number of kernels of this library the last lt_gradient_grid / lt_gradient_grid_host / lt_gradient_points call on this
+ * host thread enqueued (memsets and copies not counted): bench.py's `gpu_launches`. */
+int lt_last_launch_count(void);
 
 /*
  * Measurement hook for bench.py's roofline figure: two cudaEvent_t (as void*; both NULL switches the hook off) that the

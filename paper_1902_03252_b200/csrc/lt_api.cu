@@ -5,6 +5,8 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "../../include/lt_gradient.h"
 #include "lt_mixed.cuh"
 
@@ -16,10 +18,11 @@ namespace {
 thread_local int g_last_cuda_error = 0;
 
 struct Tuning {
-  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0;
+  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0;
 };
 Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
+thread_local int g_launches = 0;                                      // kernels launched by the last entry-point call
 
 constexpr int kDefaultChunk64 = 256;   // 32 KB of fp64 records per CTA
 constexpr int kDefaultChunk32 = 1024;  // 64 KB of fp32 records per CTA
@@ -81,15 +84,41 @@ int device_info(DeviceInfo& d) {
   return LT_OK;
 }
 
-// persistent grid: min(#work groups, resident CTAs) with the smem opt-in set
+// resident CTAs of `kernel` on the whole device with `smem` bytes of dynamic shared memory (opt-in set); cached per
+// (kernel, smem) because the two runtime queries cost microseconds on a path that launches sub-millisecond kernels
+template <class K>
+int resident_ctas(K kernel, size_t smem, const DeviceInfo& d, long long& resident) {
+  struct Entry { const void* fn; size_t smem; int device, occ; };
+  static Entry cache[32];                  // process-wide (the opt-in is a property of the function, not the thread)
+  static int n_cache = 0;
+  static std::mutex mu;
+  std::lock_guard<std::mutex> lock(mu);
+  const void* key = reinterpret_cast<const void*>(kernel);
+  int occ = 0;
+  for (int i = 0; i < n_cache; ++i)
+    if (cache[i].fn == key && cache[i].smem == smem && cache[i].device == d.device) occ = cache[i].occ;
+  if (occ == 0) {
+    if (n_cache == 32) n_cache = 0;        // full: start over (every kernel then re-opts in on its next miss)
+    size_t opted = 0;                      // within the cache's lifetime the opt-in only grows
+    for (int i = 0; i < n_cache; ++i)
+      if (cache[i].fn == key && cache[i].device == d.device && cache[i].smem > opted) opted = cache[i].smem;
+    if (smem > opted)
+      LT_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, LT_THREADS, smem));
+    if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources);
+    cache[n_cache++] = Entry{key, smem, d.device, occ};
+  }
+  if (g_tuning.ctas_per_sm > 0 && g_tuning.ctas_per_sm < occ) occ = g_tuning.ctas_per_sm;
+  resident = (long long)occ * d.sms;
+  return LT_OK;
+}
+
+// persistent grid: min(#work groups, resident CTAs)
 template <class K>
 int grid_for(K kernel, size_t smem, long long n_work, const DeviceInfo& d, int& grid) {
-  LT_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  int occ = 0;
-  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, LT_THREADS, smem));
-  if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources);
-  if (g_tuning.ctas_per_sm > 0 && g_tuning.ctas_per_sm < occ) occ = g_tuning.ctas_per_sm;
-  long long g = (long long)occ * d.sms;
+  long long g = 0;
+  const int rc = resident_ctas(kernel, smem, d, g);
+  if (rc != LT_OK) return rc;
   if (g > n_work) g = n_work;
   if (g < 1) g = 1;
   grid = (int)g;
@@ -135,58 +164,96 @@ struct GridArgs {
   int nx, ny;
 };
 
+// Launch plan shared by the fp64 and fp32 grid kernels.  All tiles cost the same, so a persistent grid of R resident CTAs
+// over n tiles runs ceil(n/R) waves and the last one may be nearly empty (config 1: 1024 tiles of 128 x 8 pixels on
+// 296 CTAs = 3.46 waves).  Each launch therefore gets a whole number of waves of the row-major tile order and the
+// ragged rest is handed to the next smaller pixels-per-thread variant (half the tile width, more resident CTAs), whose
+// waves are proportionally shorter.  fn(ppt, tiles_x, begin, end, resident_or_null): query (resident != null) or launch.
+template <class Fn>
+int launch_waves(int ppt, const GridArgs& a, Fn fn) {
+  const long long tiles_y = (a.ny + LT_TILE_H - 1) / LT_TILE_H;
+  long long begin = 0;
+  for (;;) {
+    const int tiles_x = (a.nx + 32 * ppt - 1) / (32 * ppt);
+    const long long n_tiles = tiles_x * tiles_y;
+    long long end = n_tiles;
+    if (ppt > 1 && !g_tuning.single_launch) {
+      long long resident = 0;
+      const int rc = fn(ppt, tiles_x, 0, 0, &resident);
+      if (rc != LT_OK) return rc;
+      const long long rest = n_tiles - begin;
+      if (rest % resident != 0) end = begin + rest / resident * resident;
+    }
+    if (end > begin) {
+      const int rc = fn(ppt, tiles_x, begin, end, nullptr);
+      if (rc != LT_OK) return rc;
+    }
+    if (end == n_tiles) return LT_OK;
+    const long long ty = end / tiles_x, tx = end % tiles_x;     // first tile of the rest, in the finer tiling
+    ppt >>= 1;
+    begin = ty * ((a.nx + 32 * ppt - 1) / (32 * ppt)) + 2 * tx;
+  }
+}
+
 template <int PPT, int MINB>
-int launch_f64_ppt(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out, const DeviceInfo& d, cudaStream_t st) {
+int launch_f64_ppt(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
+                   const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end, long long* resident) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
                                sizeof(LtLens<double>), d);
   const size_t smem = (size_t)chunk * sizeof(LtLens<double>);
-  const int tiles_x = (a.nx + 32 * PPT - 1) / (32 * PPT), tiles_y = (a.ny + LT_TILE_H - 1) / LT_TILE_H;
-  const long long n_tiles = (long long)tiles_x * tiles_y;
+  if (resident) return resident_ctas(lt_grad_f64_kernel<PPT, MINB>, smem, d, *resident);
   int grid = 1;
-  const int rc = grid_for(lt_grad_f64_kernel<PPT, MINB>, smem, n_tiles, d, grid);
+  const int rc = grid_for(lt_grad_f64_kernel<PPT, MINB>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  KernelEvents ke(st);
-  lt_grad_f64_kernel<PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny,
-                                                         tiles_x, (int)n_tiles, out);
+  lt_grad_f64_kernel<PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
+                                                               a.ny, tiles_x, (int)begin, (int)end, out);
   LT_CUDA(cudaGetLastError());
+  ++g_launches;
   return LT_OK;
 }
 int launch_f64(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
                const DeviceInfo& d, cudaStream_t st) {
   // 4 pixels per thread (4 independent chains, lens record loaded once per 4 interactions) at <= 128 registers, two
-  // CTAs per SM; fewer pixels per thread only for grids too small to give every SM two tiles
-  switch (pick_ppt(g_tuning.ppt64, 4, a.nx, a.ny, d)) {
-    case 1: return launch_f64_ppt<1, 4>(l64, t64, a, out, d, st);
-    case 2: return launch_f64_ppt<2, 3>(l64, t64, a, out, d, st);
-    default: return launch_f64_ppt<4, 2>(l64, t64, a, out, d, st);
-  }
+  // CTAs per SM; fewer pixels per thread for the ragged rest and for grids too small to give every SM two tiles
+  KernelEvents ke(st);
+  return launch_waves(pick_ppt(g_tuning.ppt64, 4, a.nx, a.ny, d), a,
+                      [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
+                        switch (ppt) {
+                          case 1: return launch_f64_ppt<1, 4>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                          case 2: return launch_f64_ppt<2, 3>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                          default: return launch_f64_ppt<4, 2>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                        }
+                      });
 }
 
 template <int PPT>
-int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32,
-                   const GridArgs& a, float2* out,
-                   const DeviceInfo& d, cudaStream_t st, bool hook) {
+int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32, const GridArgs& a,
+                   float2* out, const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end,
+                   long long* resident) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
                                sizeof(LtLens<float>), d);
   const size_t smem = (size_t)chunk * sizeof(LtLens<float>);
-  const int tiles_x = (a.nx + 32 * PPT - 1) / (32 * PPT), tiles_y = (a.ny + LT_TILE_H - 1) / LT_TILE_H;
-  const long long n_tiles = (long long)tiles_x * tiles_y;
+  if (resident) return resident_ctas(lt_grad_f32_kernel<PPT>, smem, d, *resident);
   int grid = 1;
-  const int rc = grid_for(lt_grad_f32_kernel<PPT>, smem, n_tiles, d, grid);
+  const int rc = grid_for(lt_grad_f32_kernel<PPT>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  KernelEvents ke(st, hook);
   lt_grad_f32_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
-                                                         a.ny, tiles_x, (int)n_tiles, out);
+                                                         a.ny, tiles_x, (int)begin, (int)end, out);
   LT_CUDA(cudaGetLastError());
+  ++g_launches;
   return LT_OK;
 }
 int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32, const GridArgs& a,
                float2* out, const DeviceInfo& d, cudaStream_t st, bool hook = true) {
-  switch (pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d)) {
-    case 1: return launch_f32_ppt<1>(l64, l32, t32, a, out, d, st, hook);
-    case 2: return launch_f32_ppt<2>(l64, l32, t32, a, out, d, st, hook);
-    default: return launch_f32_ppt<4>(l64, l32, t32, a, out, d, st, hook);
-  }
+  KernelEvents ke(st, hook);
+  return launch_waves(pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d), a,
+                      [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
+                        switch (ppt) {
+                          case 1: return launch_f32_ppt<1>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          case 2: return launch_f32_ppt<2>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          default: return launch_f32_ppt<4>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                        }
+                      });
 }
 
 template <bool FROM_LIST>
@@ -203,6 +270,7 @@ int launch_list(const LtLens<double>* l64, const LtTables<double>* t64, const Gr
   lt_grad_list_f64_kernel<FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
                                                                     a.nx, list, hdr, points, n_points, out);
   LT_CUDA(cudaGetLastError());
+  ++g_launches;
   return LT_OK;
 }
 
@@ -224,6 +292,7 @@ int precompute(const lt_lens* d_lenses, int n_lens, double dx, unsigned char* ws
                                                reinterpret_cast<LtTables<float>*>(ws + L.tab32),
                                                reinterpret_cast<LtWsHeader*>(ws + L.header));
   LT_CUDA(cudaGetLastError());
+  ++g_launches;
   return LT_OK;
 }
 
@@ -282,8 +351,11 @@ void lt_mixed_defaults(lt_mixed_params* out) {
   out->b0_cluster_threshold = 15.0;        /* R15 */
 }
 
-int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm) {
-  if (ppt64 < 0 || ppt32 < 0 || chunk64 < 0 || chunk32 < 0 || ctas_per_sm < 0) return LT_ERR_BAD_SIZE;
+int lt_last_launch_count(void) { return g_launches; }
+
+int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm, int single_launch) {
+  if (ppt64 < 0 || ppt32 < 0 || chunk64 < 0 || chunk32 < 0 || ctas_per_sm < 0 || single_launch < 0) return LT_ERR_BAD_SIZE;
+  g_tuning.single_launch = single_launch;
   g_tuning.ppt64 = ppt64;
   g_tuning.ppt32 = ppt32;
   g_tuning.chunk64 = chunk64;
@@ -326,6 +398,7 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y
   DeviceInfo dev;
   int rc = device_info(dev);
   if (rc != LT_OK) return rc;
+  g_launches = 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   unsigned char* ws = (unsigned char*)d_workspace;
   LtWsHeader* hdr = reinterpret_cast<LtWsHeader*>(ws + L.header);
@@ -356,6 +429,7 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y
     lt_patch_kernel<<<n_lens, 256, 0, st>>>(reinterpret_cast<const LtRawLens*>(d_lenses), n_lens, x_min, y_min, dx,
                                             nx, ny, md, flags);
     LT_CUDA(cudaGetLastError());
+    ++g_launches;
   }
   rc = launch_f32(l64, l32, t32, a, sp, dev, st, /*hook=*/false);
   if (rc != LT_OK) return rc;
@@ -365,6 +439,7 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y
     if (blocks > cap) blocks = cap;
     lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, (double2*)d_out_grad, list, hdr);   /* a8 */
     LT_CUDA(cudaGetLastError());
+    ++g_launches;
   }
   return launch_list<true>(l64, t64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
 }
@@ -379,6 +454,7 @@ int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_poin
   DeviceInfo dev;
   int rc = device_info(dev);
   if (rc != LT_OK) return rc;
+  g_launches = 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   unsigned char* ws = (unsigned char*)d_workspace;
   rc = precompute(d_lenses, n_lens, 1.0, ws, L, st);

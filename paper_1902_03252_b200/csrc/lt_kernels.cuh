@@ -6,7 +6,9 @@
 // warp is one contiguous 512 B / 256 B line), walks the lens catalogue staged in shared memory in chunks (every lane
 // reads the same record: broadcast LDS.128, no bank conflicts), keeps the 2*PPT accumulators in registers for the whole
 // lens loop (Alg. 1 l.13-14) and stores each pixel once.  The grid is persistent: min(#tiles, CTAs/SM * #SM) CTAs
-// stride over the tiles, so a catalogue that fits one chunk is staged once per CTA (fp64).
+// stride over the tiles [tile_begin, tile_end) of the row-major tile order, so a catalogue that fits one chunk is
+// staged once per CTA (fp64).  The host (lt_api.cu) gives each launch a whole number of waves and hands the ragged
+// rest to the next smaller pixels-per-thread variant.
 #pragma once
 #include <cuda_runtime.h>
 #include "lt_pack.cuh"
@@ -62,8 +64,8 @@ __device__ __forceinline__ void lt_copy16(void* dst, const void* src, int count)
 template <int PPT, int MINB>
 __global__ void __launch_bounds__(LT_THREADS, MINB)
 lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<double>* __restrict__ tables, int n_lens,
-                   int chunk, double x_min, double y_min, double dx, int nx, int ny, int tiles_x, int n_tiles,
-                   double2* __restrict__ out) {
+                   int chunk, double x_min, double y_min, double dx, int nx, int ny, int tiles_x, int tile_begin,
+                   int tile_end, double2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
   __shared__ LtTables<double> tab;
   LtLens<double>* sl = reinterpret_cast<LtLens<double>*>(lt_smem);
@@ -76,7 +78,7 @@ lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<doubl
     lt_copy16(sl, lens, n_lens * (int)(sizeof(LtLens<double>) / 16));
     __syncthreads();
   }
-  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+  for (int tile = tile_begin + blockIdx.x; tile < tile_end; tile += gridDim.x) {
     const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
     const int j = ty * LT_TILE_H + wrp;
     const int i0 = tx * TILE_W + lane;
@@ -125,7 +127,7 @@ template <int PPT>
 __global__ void __launch_bounds__(LT_THREADS)
 lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float>* __restrict__ lens32,
                    const LtTables<float>* __restrict__ tables, int n_lens, int chunk, double x_min, double y_min,
-                   double dx, int nx, int ny, int tiles_x, int n_tiles, float2* __restrict__ out) {
+                   double dx, int nx, int ny, int tiles_x, int tile_begin, int tile_end, float2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
   __shared__ LtTables<float> tab;
   LtLens<float>* sl = reinterpret_cast<LtLens<float>*>(lt_smem);
@@ -137,7 +139,7 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
   float il[PPT];
 #pragma unroll
   for (int p = 0; p < PPT; ++p) il[p] = (float)(lane + 32 * p) - 0.5f * (float)(TILE_W - 1);
-  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+  for (int tile = tile_begin + blockIdx.x; tile < tile_end; tile += gridDim.x) {
     const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
     const int j = ty * LT_TILE_H + wrp;
     const int i0 = tx * TILE_W + lane;

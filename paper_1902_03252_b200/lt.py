@@ -21,7 +21,7 @@ _LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
 
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
-           "lt_set_tuning", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
+           "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
 
 
 class lt_mixed_params(ctypes.Structure):
@@ -71,7 +71,8 @@ def lib():
         L.lt_gradient_grid_host.restype = ci
         L.lt_gradient_points.argtypes = [vp, ci, vp, cll, vp, vp, sz, vp]
         L.lt_gradient_points.restype = ci
-        L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci]
+        L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci, ci]
+        L.lt_last_launch_count.restype = ci
         L.lt_set_tuning.restype = ci
         L.lt_set_kernel_events.argtypes = [vp, vp]
         L.lt_set_kernel_events.restype = ci
@@ -132,8 +133,13 @@ def lt_host_workspace_bytes(n_lens, nx, ny, mode):
     return int(lib().lt_host_workspace_bytes(int(n_lens), int(nx), int(ny), int(mode)))
 
 
-def lt_set_tuning(ppt64=0, ppt32=0, chunk64=0, chunk32=0, ctas_per_sm=0):
-    _check(lib().lt_set_tuning(int(ppt64), int(ppt32), int(chunk64), int(chunk32), int(ctas_per_sm)), "lt_set_tuning")
+def lt_set_tuning(ppt64=0, ppt32=0, chunk64=0, chunk32=0, ctas_per_sm=0, single_launch=0):
+    _check(lib().lt_set_tuning(int(ppt64), int(ppt32), int(chunk64), int(chunk32), int(ctas_per_sm),
+                               int(single_launch)), "lt_set_tuning")
+
+
+def lt_last_launch_count():
+    return int(lib().lt_last_launch_count())
 
 
 def lt_set_kernel_events(ev_start=None, ev_stop=None):

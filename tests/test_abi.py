@@ -75,7 +75,7 @@ def test_argument_errors_need_no_gpu(L):
     bad = L.lt_mixed_params(-1.0, 0.3, 6.0, 0.3, 15.0)
     assert lib.lt_gradient_grid(vp(16), 4, 0.0, 0.0, 1.0, 8, 8, 2, ctypes.byref(bad), vp(16), vp(16), 1 << 20, None) == -7
     assert lib.lt_gradient_points(vp(16), 4, vp(16), -1, vp(16), vp(16), 1 << 20, None) == -2
-    assert lib.lt_set_tuning(-1, 0, 0, 0, 0) == -2 and lib.lt_set_tuning(0, 0, 0, 0, 0) == 0
+    assert lib.lt_set_tuning(-1, 0, 0, 0, 0, 0) == -2 and lib.lt_set_tuning(0, 0, 0, 0, 0, 0) == 0
 
 
 def test_binding_refuses_cpu_tensors(L):

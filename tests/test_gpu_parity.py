@@ -92,6 +92,39 @@ def test_launch_configurations_agree(env, ppt64, ppt32, chunk):
     assert _err(a, ref) < TOL_F64 and _err(b, ref) < TOL_F32
 
 
+@pytest.mark.parametrize("nx,ny,ctas", [(1500, 1111, 0), (1027, 2049, 1), (4096, 300, 2), (129, 4100, 0)])
+def test_wave_split_covers_every_pixel_once(env, nx, ny, ctas):
+    """The launch plan (whole waves of the widest variant, ragged rest to the finer ones: lt_api.cu launch_waves)
+    writes every pixel exactly as the single-launch plan does: fp64 bit-equal, fp32 within tolerance, no pixel left
+    unwritten (the output is poisoned with NaN first)."""
+    torch, lt, O = env
+    W = workloads.make(0)
+    L = torch.from_numpy(W.lenses[:3].copy()).cuda()
+    x_min, y_min, dx = -40.0, -31.0, 0.05
+    res = {}
+    for single in (1, 0):
+        for mode, dt in ((lt.LT_FP64, torch.float64), (lt.LT_FP32, torch.float32)):
+            out = torch.full((ny, nx, 2), float("nan"), dtype=dt, device="cuda")
+            try:
+                lt.lt_set_tuning(0, 0, 0, 0, ctas, single)
+                lt.lt_gradient_grid(L, x_min, y_min, dx, nx, ny, mode, out=out)
+                n_launch = lt.lt_last_launch_count()
+            finally:
+                lt.lt_set_tuning()
+            torch.cuda.synchronize()
+            assert not torch.isnan(out).any()
+            assert n_launch == 2 if single else n_launch >= 2
+            res[(single, mode)] = out.cpu().numpy()
+    assert np.array_equal(res[(0, lt.LT_FP64)], res[(1, lt.LT_FP64)])
+    s = np.abs(res[(1, lt.LT_FP64)]).max()
+    assert np.abs(res[(0, lt.LT_FP32)].astype(np.float64) - res[(1, lt.LT_FP64)]).max() / s < TOL_F32
+    # a sample of pixels against the oracle (the rest is covered by the equality above)
+    rng = np.random.default_rng(7)
+    i, j = rng.integers(0, nx, 500), rng.integers(0, ny, 500)
+    ref = O.gradient_points(W.lenses[:3], x_min + i * dx, y_min + j * dx)
+    assert np.abs(res[(0, lt.LT_FP64)][j, i] - ref).max() / np.abs(ref).max() < TOL_F64
+
+
 def test_full_size_cfg1_sampled_and_points(env):
     """BASELINE config 1 at full size, in the launch configuration bench.py times: sampled pixels (random + the pixels
     nearest every lens centre) against the oracle, and lt_gradient_points against the grid kernel (bit-equal)."""
