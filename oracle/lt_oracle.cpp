@@ -20,7 +20,8 @@
  *               whose convergence is kappa = (b0/2) rcut/(rcut-rcore) [1/sqrt(rcore^2+rho^2) - 1/sqrt(rcut^2+rho^2)]
  *               (alpha = grad psi, laplace psi = 2 kappa: eq. 2-4).
  *   circular  : e < 1e-14: north star's closed form
- *               alpha(R) = b0 rcut/(rcut-rcore) [(sqrt(rcore^2+R^2)-rcore) - (sqrt(rcut^2+R^2)-rcut)] / R, along (x,y)/R.
+ *               alpha(R) = b0 rcut/(rcut-rcore) [(sqrt(rcore^2+R^2)-rcore) - (sqrt(rcut^2+R^2)-rcut)] / R, along (x,y)/R,
+ *               each bracket evaluated as R^2/(sqrt(w^2+R^2)+w) (reading R22: identical value, no cancellation).
  *   mixed rule: section 3.3, eq. 24-28 and the DP centre patches of section 3.2, with the
  *               readings R11-R16 of DESIGN.md (thresholds scaled with the pixel size).
  *
@@ -120,7 +121,10 @@ void dpie_body(T x, T y, T e, T rcore, T rcut, T b0, bool reflect, T& gx, T& gy)
     const T R2 = x * x + y * y;
     const T R = M<T>::sqrt_(R2);
     if (R == T(0)) { gx = T(0); gy = T(0); return; }      /* reading R5 */
-    const T a = b0 * scale * ((M<T>::sqrt_(rcore * rcore + R2) - rcore) - (M<T>::sqrt_(rcut * rcut + R2) - rcut)) / R;
+    /* sqrt(w^2+R^2) - w written as R^2 / (sqrt(w^2+R^2) + w): the same number without the cancellation that costs the
+     * literal form ulp(w)/R at R << w (reading R22; pinned against the literal form in __float128) */
+    const T hc = R2 / (M<T>::sqrt_(rcore * rcore + R2) + rcore), ht = R2 / (M<T>::sqrt_(rcut * rcut + R2) + rcut);
+    const T a = b0 * scale * (hc - ht) / R;
     gx = a * x / R; gy = a * y / R;
     return;
   }

@@ -106,6 +106,22 @@ def test_circular_closed_form_central_slope_and_far_field():
         assert abs(v[0] / v[1] - 0.75) < 1e-6      # radial
 
 
+def test_circular_closed_form_small_radius_series():
+    """Reading R22: for R << rcore the closed form has the series b0 R/(2 rcore) - b0 s R^3/8 (1/rcore^3 - 1/rcut^3) + O(R^5),
+    s = rcut/(rcut-rcore) (from sqrt(w^2+R^2) - w = R^2/2w - R^4/8w^3 + ...).  The literal difference of square roots
+    loses ulp(rcut)/R there (1e-6 relative at R = 1e-5, rcut = 1000 even in long double); the oracle's rearranged
+    evaluation must meet the series to fp64 rounding."""
+    b0, rc, rt = 7.0, 0.4, 1000.0
+    L = np.array([[0.0, 0.0, 0.0, 0.0, rc, rt, b0]])
+    for R in (1e-5, 1e-4, 1e-3):
+        v = O.gradient_points(L, [R * 0.6], [-R * 0.8])[0]
+        series = b0 * R / (2 * rc) - b0 * rt / (rt - rc) * R ** 3 / 8 * (1 / rc ** 3 - 1 / rt ** 3)
+        assert abs(np.hypot(*v) / series - 1) < 5e-16 + (R / rc) ** 4
+        assert abs(v[0] / v[1] + 0.75) < 1e-15
+        q = O.gradient_points(L, [R * 0.6], [-R * 0.8], O.QUAD)[0]
+        assert np.abs(v - q).max() / np.abs(q).max() < 3e-16
+
+
 def test_div_is_2kappa_and_curl_is_zero():
     """4th-order central differences of the oracle's own alpha: div = 2 kappa (elementary expression), curl = 0."""
     W = workloads.make(0)
