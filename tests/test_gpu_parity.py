@@ -241,3 +241,31 @@ def test_host_buffer_entry_point(env):
         lt.lt_gradient_grid_host(hL, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, hout, ws)
         torch.cuda.synchronize()
         assert np.array_equal(hout.numpy(), _gpu_map(torch, lt, W, mode))
+
+
+def test_row_block_sharding_stitches_to_the_unsharded_map(env):
+    """DESIGN.md section 9 on one GPU: the row blocks two ranks would compute (shard.compute_block through the real
+    lt_gradient_grid; mixed with its self-computed halo row) stitched together against the unsharded map and the oracle."""
+    torch, lt, O = env
+    from paper_1902_03252_b200 import shard
+    W = workloads.make(1, paper_regime=True, n_override=301)
+    L = torch.from_numpy(W.lenses).cuda()
+    ref = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny)
+    s = np.abs(ref).max()
+
+    def compute(lenses, x_min, y_min, dx, nx, ny, mode):
+        return lt.lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode)
+    for mode, tol in ((lt.LT_FP64, TOL_F64), (lt.LT_FP32, TOL_F32), (lt.LT_MIXED, TOL_F32)):
+        whole = _gpu_map(torch, lt, W, mode).astype(np.float64)
+        for world in (2, 3):
+            parts = []
+            for rank in range(world):
+                b, out = shard.compute_block(compute, L, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, rank, world,
+                                             mixed_mode=lt.LT_MIXED)
+                assert out.shape[0] == b.j1 - b.j0
+                parts.append(out.cpu().numpy().astype(np.float64))
+            stitched = np.concatenate(parts, axis=0)
+            assert stitched.shape == whole.shape
+            assert np.abs(stitched - ref).max() / s < tol
+            # blocks differ from the unsharded call by the rounding of their first row's coordinate only
+            assert np.abs(stitched - whole).max() / s < (1e-13 if mode == lt.LT_FP64 else tol)
