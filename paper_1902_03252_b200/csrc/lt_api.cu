@@ -226,18 +226,18 @@ int launch_f64(const LtLens<double>* l64, const LtTables<double>* t64, const Gri
                       });
 }
 
-template <int PPT>
+template <int PPT, int MINB>
 int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32, const GridArgs& a,
                    float2* out, const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end,
                    long long* resident) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
                                sizeof(LtLens<float>), d);
   const size_t smem = (size_t)chunk * sizeof(LtLens<float>);
-  if (resident) return resident_ctas(lt_grad_f32_kernel<PPT>, smem, d, *resident);
+  if (resident) return resident_ctas(lt_grad_f32_kernel<PPT, MINB>, smem, d, *resident);
   int grid = 1;
-  const int rc = grid_for(lt_grad_f32_kernel<PPT>, smem, end - begin, d, grid);
+  const int rc = grid_for(lt_grad_f32_kernel<PPT, MINB>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  lt_grad_f32_kernel<PPT><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
+  lt_grad_f32_kernel<PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
                                                          a.ny, tiles_x, (int)begin, (int)end, out);
   LT_CUDA(cudaGetLastError());
   ++g_launches;
@@ -245,13 +245,15 @@ int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const Lt
 }
 int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32, const GridArgs& a,
                float2* out, const DeviceInfo& d, cudaStream_t st, bool hook = true) {
+  // 4 pixels per thread at <= 80 registers (3 CTAs per SM): with a tighter register budget the compiler reloads the
+  // constants inside the loop and the kernel, which is bound by issue slots, loses 10 %
   KernelEvents ke(st, hook);
   return launch_waves(pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
                         switch (ppt) {
-                          case 1: return launch_f32_ppt<1>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
-                          case 2: return launch_f32_ppt<2>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
-                          default: return launch_f32_ppt<4>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          case 1: return launch_f32_ppt<1, 6>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          case 2: return launch_f32_ppt<2, 4>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          default: return launch_f32_ppt<4, 3>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
                         }
                       });
 }

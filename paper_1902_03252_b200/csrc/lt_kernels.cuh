@@ -123,8 +123,8 @@ lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<doubl
 //   x' = X0 + il*(dx cos) + jl*(dx sin),  y' = Y0 + jl*(dx cos) - il*(dx sin)      (Alg. 1 l.3-6 merged)
 // so the fp32 rounding of the coordinate is relative to the tile size, not to |theta| (the |theta_c|/|dtheta| term of
 // (A.65)).  All per-interaction arithmetic is FP32.
-template <int PPT>
-__global__ void __launch_bounds__(LT_THREADS)
+template <int PPT, int MINB>
+__global__ void __launch_bounds__(LT_THREADS, MINB)
 lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float>* __restrict__ lens32,
                    const LtTables<float>* __restrict__ tables, int n_lens, int chunk, double x_min, double y_min,
                    double dx, int nx, int ny, int tiles_x, int tile_begin, int tile_end, float2* __restrict__ out) {
