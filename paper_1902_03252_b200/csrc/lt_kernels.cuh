@@ -190,11 +190,66 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
 }
 
 // ------------------------------------------------------------------------------------------------ fp64 list kernel
-// One pixel per thread, pixels taken from (a) the compacted list of flagged pixel indices of the mixed rule (a9;
-// count read from the workspace header on the device, no host round trip) or (b) an array of arbitrary points.
-// Uses the same lt_interaction in the same lens order as the fp64 grid kernel: identical bits for identical pixels.
+// Pixels taken from (a) the compacted list of flagged pixel indices of the mixed rule (a9; count read from the
+// workspace header on the device, no host round trip) or (b) an array of arbitrary points.  Uses the same
+// lt_interaction in the same lens order as the fp64 grid kernel: identical bits for identical pixels.
+// Groups of 4 * 256 entries, 4 per thread (entries 256 apart, so list reads stay coalesced); a rest of at most one
+// 256-entry group per CTA after the whole waves runs one entry per thread (the count is only known on the device, so
+// the split is made here, not on the host).
+template <bool FROM_LIST, int PPT>
+__device__ __forceinline__ void lt_list_group(const LtLens<double>* __restrict__ lens, const LtLens<double>* sl,
+                                              const LtTables<double>& tab, int n_lens, int chunk, bool single,
+                                              double x_min, double y_min, double dx, int nx,
+                                              const unsigned int* __restrict__ list,
+                                              const double2* __restrict__ points, long long first, long long total,
+                                              double2* __restrict__ out) {
+  double t1[PPT], t2[PPT], G1[PPT], G2[PPT];
+  size_t dst[PPT];
+  bool live[PPT];
+#pragma unroll
+  for (int p = 0; p < PPT; ++p) {
+    const long long t = first + (long long)p * LT_THREADS + threadIdx.x;
+    live[p] = t < total;
+    t1[p] = 0.0; t2[p] = 0.0; dst[p] = 0; G1[p] = 0.0; G2[p] = 0.0;
+    if (live[p]) {
+      if (FROM_LIST) {
+        const unsigned int pix = list[t];
+        const int j = (int)(pix / (unsigned int)nx), i = (int)(pix - (unsigned int)j * (unsigned int)nx);
+        t1[p] = __dadd_rn(x_min, __dmul_rn((double)i, dx));
+        t2[p] = __dadd_rn(y_min, __dmul_rn((double)j, dx));
+        dst[p] = pix;
+      } else {
+        const double2 pt = points[t];
+        t1[p] = pt.x;
+        t2[p] = pt.y;
+        dst[p] = (size_t)t;
+      }
+    }
+  }
+  for (int base = 0; base < n_lens; base += chunk) {
+    const int cnt = min(chunk, n_lens - base);
+    if (!single) {
+      __syncthreads();
+      lt_copy16(const_cast<LtLens<double>*>(sl), lens + base, cnt * (int)(sizeof(LtLens<double>) / 16));
+      __syncthreads();
+    }
+#pragma unroll 1
+    for (int k = 0; k < cnt; ++k) {
+      const LtLens<double> L = sl[k];
+#pragma unroll
+      for (int p = 0; p < PPT; ++p) {
+        const double d2 = t2[p] - L.y0;
+        lt_interaction<double>(t1[p] - L.x0, d2 * L.sx, d2 * L.cy, L, tab, G1[p], G2[p]);
+      }
+    }
+  }
+#pragma unroll
+  for (int p = 0; p < PPT; ++p)
+    if (live[p]) out[dst[p]] = make_double2(G1[p], G2[p]);
+}
+
 template <bool FROM_LIST>
-__global__ void __launch_bounds__(LT_THREADS)
+__global__ void __launch_bounds__(LT_THREADS, 2)
 lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<double>* __restrict__ tables,
                         int n_lens, int chunk, double x_min, double y_min, double dx, int nx,
                         const unsigned int* __restrict__ list, const LtWsHeader* __restrict__ hdr,
@@ -210,41 +265,19 @@ lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<
     lt_copy16(sl, lens, n_lens * (int)(sizeof(LtLens<double>) / 16));
     __syncthreads();
   }
-  const long long n_groups = (total + LT_THREADS - 1) / LT_THREADS;
-  for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
-    const long long t = g * LT_THREADS + threadIdx.x;
-    const bool live = t < total;
-    double t1 = 0.0, t2 = 0.0;
-    size_t dst = 0;
-    if (live) {
-      if (FROM_LIST) {
-        const unsigned int pix = list[t];
-        const int j = (int)(pix / (unsigned int)nx), i = (int)(pix - (unsigned int)j * (unsigned int)nx);
-        t1 = __dadd_rn(x_min, __dmul_rn((double)i, dx));
-        t2 = __dadd_rn(y_min, __dmul_rn((double)j, dx));
-        dst = pix;
-      } else {
-        const double2 pt = points[t];
-        t1 = pt.x;
-        t2 = pt.y;
-        dst = (size_t)t;
-      }
-    }
-    double G1 = 0.0, G2 = 0.0;
-    for (int base = 0; base < n_lens; base += chunk) {
-      const int cnt = min(chunk, n_lens - base);
-      if (!single) {
-        __syncthreads();
-        lt_copy16(sl, lens + base, cnt * (int)(sizeof(LtLens<double>) / 16));
-        __syncthreads();
-      }
-#pragma unroll 1
-      for (int k = 0; k < cnt; ++k) {
-        const LtLens<double> L = sl[k];
-        const double d2 = t2 - L.y0;
-        lt_interaction<double>(t1 - L.x0, d2 * L.sx, d2 * L.cy, L, tab, G1, G2);
-      }
-    }
-    if (live) out[dst] = make_double2(G1, G2);
+  constexpr int WIDE = 4;
+  const long long per_wave = (long long)gridDim.x * (WIDE * LT_THREADS);
+  long long n_wide = total / per_wave * gridDim.x;                  // groups of WIDE * 256 entries: whole waves
+  long long rest0 = n_wide * (WIDE * LT_THREADS);
+  if (total - rest0 > (long long)gridDim.x * LT_THREADS) {          // more than one narrow group per CTA left:
+    n_wide = (total + WIDE * LT_THREADS - 1) / (WIDE * LT_THREADS); // a ragged wide wave is cheaper than narrow rounds
+    rest0 = total;
   }
+  for (long long g = blockIdx.x; g < n_wide; g += gridDim.x)
+    lt_list_group<FROM_LIST, WIDE>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
+                                   g * (WIDE * LT_THREADS), total, out);
+  const long long n_rest = (total - rest0 + LT_THREADS - 1) / LT_THREADS;   // <= gridDim.x
+  for (long long g = blockIdx.x; g < n_rest; g += gridDim.x)
+    lt_list_group<FROM_LIST, 1>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
+                                rest0 + g * LT_THREADS, total, out);
 }
