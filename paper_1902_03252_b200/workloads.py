@@ -105,3 +105,47 @@ def random_catalogue(seed, n_lens, L=50.0, e_max=0.6):
     out = _galaxies(rng, n_lens, lambda: (rng.uniform(-L, L), rng.uniform(-L, L)))
     out[:, 2] *= e_max / 0.6
     return out
+
+
+# ---------------------------------------------------------------------------------------------- SIE (the paper's body)
+# A catalogue of SIE lenses is a float64 array [n_lens, 5]: (xc, yc, epsilon, Phi, b0) = `lt_sie_lens`.
+ARCSEC_PER_RAD = 206264.80624709636
+C_KM_S = 299792.458
+
+
+def b0_from_sigma_v(sigma_km_s):
+    """eq. 22: b0 = 4 pi (sigma_v / c)^2, converted from radians to arcsec (D_LS/D_OS = 1)."""
+    return 4.0 * np.pi * (np.asarray(sigma_km_s, dtype=np.float64) / C_KM_S) ** 2 * ARCSEC_PER_RAD
+
+
+def make_sie(kind="paper", n_override=None, seed_offset=0):
+    """Synthetic stand-in for the paper's benchmark (section 4): 6730 x 6730 pixels at 0.03"/pixel, two
+    cluster-scale SIE halos (sigma_v = 1000 and 700 km/s, epsilon = 0.05 and 0.04) and 700 galaxy-scale halos (sigma_v
+    uniform in 10-15 km/s, epsilon uniform in 0-0.15).  The paper gives no positions or angles: cluster centres are
+    drawn uniform in [-20,20]^2, galaxy centres Gaussian (sigma 40") redrawn until inside the grid, angles uniform in
+    [0, pi).  kind = "small": 96 x 96 pixels over the same extent and 2 + 30 halos (the oracle finishes in well under
+    a second).  n_override: n x n pixels over the same extent."""
+    if kind == "paper":
+        name, n, n_gal, seed = "sie_paper_6730x6730_702", 6730, 700, 2000
+    elif kind == "small":
+        name, n, n_gal, seed = "sie_small_96x96_32", 96, 30, 2001
+    else:
+        raise ValueError("kind must be 'paper' or 'small'")
+    L = 0.5 * 6730 * 0.03
+    seed += int(seed_offset)
+    rng = np.random.default_rng(seed)
+    if n_override is not None:
+        n = int(n_override)
+        name += "_n%d" % n
+    x_min, y_min, dx = grid(n, L)
+    out = np.empty((2 + n_gal, 5))
+    for k, (sig, eps) in enumerate(((1000.0, 0.05), (700.0, 0.04))):
+        out[k] = (rng.uniform(-20, 20), rng.uniform(-20, 20), eps, rng.uniform(0.0, np.pi), b0_from_sigma_v(sig))
+    for k in range(n_gal):                     # fixed draw order per lens: centre, sigma_v, epsilon, Phi
+        while True:
+            xc, yc = rng.normal(0.0, 40.0, 2)
+            if abs(xc) < L and abs(yc) < L:
+                break
+        sig = rng.uniform(10.0, 15.0)
+        out[2 + k] = (xc, yc, rng.uniform(0.0, 0.15), rng.uniform(0.0, np.pi), b0_from_sigma_v(sig))
+    return Workload(name, out, x_min, y_min, dx, n, n, seed)
