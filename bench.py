@@ -18,6 +18,10 @@ N > 1 (torchrun, one rank per GPU): the path shards with no exchange (pixels and
 P:98): every rank computes the full map of its OWN catalogue (seed + rank) -- weak scaling, no collective
 on the data path; NCCL is used only for the barrier and the max over ranks.
 
+--model sie: the same path with the paper's own lens body (Algorithm 1) on a synthetic stand-in for the paper's benchmark
+(6730 x 6730 pixels at 0.03", 2 cluster-scale + 700 galaxy-scale SIE halos); `vs_baseline` is then the ratio to
+the paper's V100 throughput derived from Table 2 -- another machine's number, context only.
+
 --impl reference: times the CPU oracle (oracle/lt_oracle.cpp, `double` instantiation, as it stands) on the host cores,
 each step a bounded row sample of the same workload; rank 0 only.
 """
@@ -40,6 +44,11 @@ DTYPE = {"fp64": "f64", "fp32": "f32", "mixed": "f32+f64"}
 # FLOP-count convention per lens-pixel interaction (DESIGN.md section 8 / SURVEY 8(d)): textbook evaluation with
 # per-lens constants precomputed, add/sub/mul = 1, FMA = 2: 61 flops + 8 specials (2 sqrt, 2 div, 2 ln, 2 atan2).
 F_NOM = 69.0
+# SIE (Algorithm 1) under the same convention: translate 2 + rotate 6 + R^2 5 + g 4 (with (1 -+ eps) b0
+# precomputed: 2 mul, 2 div by R counted as mul by 1/R) + rotate back 6 + accumulate 2 = 25 flops + 1 rsqrt.
+F_NOM_SIE = 26.0
+# the paper's own numbers for the SIE benchmark workload (Table 2 P:364-373 -> BASELINE.md, derived throughput on V100)
+PAPER_V100_SIE = {"fp64": 6.9e10, "mixed": 8.2e10}
 # lanes per SM behind the "alu" peaks (paper's Table 1 convention: 2 ops/cycle x clock x lanes)
 LANES = {"fp64": 64, "fp32": 128, "mixed": 64}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at config 1, from the ncu --set full
@@ -57,6 +66,9 @@ def parse_args():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = the metric's)")
     ap.add_argument("--mode", default="fp64", choices=list(MODES))
     ap.add_argument("--paper-regime", action="store_true", help="light galaxy halos (DESIGN.md section 4)")
+    ap.add_argument("--model", default="dpie", choices=["dpie", "sie"],
+                    help="dpie: BASELINE.json configs (headline); sie: the paper's Algorithm 1 on its benchmark "
+                         "workload, 6730^2 pixels x 702 halos (SURVEY 8(f) NEXT-1)")
     ap.add_argument("--no-extras", action="store_true", help="skip the other modes, cpu_baseline and peak probes")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU work of the oracle sample")
     return ap.parse_args()
@@ -137,14 +149,24 @@ def measured_peaks():
 # ------------------------------------------------------------------------------------------------ reference arm
 def oracle_sample(W, cpu_seconds, ns_per_interaction=100.0):
     """Row stride so that the `double` oracle does about `cpu_seconds` of CPU work on this workload."""
+    if W.lenses.shape[1] == 5:
+        ns_per_interaction = 15.0                 # SIE: one sqrt, two divisions
     total = W.nx * W.ny * len(W.lenses) * ns_per_interaction * 1e-9
     stride = max(1, int(round(total / cpu_seconds)))
     rows = (W.ny + stride - 1) // stride
     return stride, rows
 
 
+def oracle_module(W):
+    if W.lenses.shape[1] == 5:
+        from oracle import lt_oracle_sie as O
+    else:
+        from oracle import lt_oracle as O
+    return O
+
+
 def time_oracle(W, stride, threads=0):
-    from oracle import lt_oracle as O
+    O = oracle_module(W)
     O.lib()
     t0 = time.perf_counter()
     O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, precision=O.DOUBLE, n_threads=threads,
@@ -158,8 +180,8 @@ def run_reference(args, W):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle import lt_oracle as O
-    cores = O.max_threads()
+    from oracle import lt_oracle as O0
+    cores = O0.max_threads()
     # every step = one bounded sample; the whole run (warmup + steps) is sized to stay within ~2 minutes of wall time
     budget = 100.0 * cores / max(1, args.steps + args.warmup)
     stride, rows = oracle_sample(W, min(args.cpu_seconds, budget))
@@ -193,6 +215,11 @@ class Runner:
         self.torch, self.lt, self.W, self.mode = torch, lt, W, mode
         self.code = MODES[mode]
         n = len(W.lenses)
+        self.sie = W.lenses.shape[1] == 5
+        self.grid = lt.lt_gradient_grid_sie if self.sie else lt.lt_gradient_grid
+        self.grid_host = lt.lt_gradient_grid_sie_host if self.sie else lt.lt_gradient_grid_host
+        # SIE: the paper's rule at its own pixel size; cluster-scale = b0 >= 1" (its cluster halos: 28.8", 14.1")
+        self.mixed = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0) if self.sie else None
         self.d_lenses = torch.from_numpy(W.lenses).cuda()
         dt = torch.float32 if mode == "fp32" else torch.float64
         self.out = torch.empty((W.ny, W.nx, 2), dtype=dt, device="cuda")
@@ -202,18 +229,19 @@ class Runner:
         self.ws_host = lt.alloc_workspace(n, W.nx, W.ny, self.code, host=True)
         self.units = W.nx * W.ny * n
         self.h2d = self.h_lenses.numel() * 8
+        self.f_nom = F_NOM_SIE if self.sie else F_NOM
         self.d2h = self.h_out.numel() * self.h_out.element_size()
 
     def step(self):
         W = self.W
-        self.lt.lt_gradient_grid(self.d_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, out=self.out,
-                                 workspace=self.ws)
+        self.grid(self.d_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, mixed=self.mixed, out=self.out,
+                  workspace=self.ws)
         self.launches = self.lt.lt_last_launch_count()      # kernels of ours this step enqueued (memsets not counted)
 
     def step_host(self):
         W = self.W
-        self.lt.lt_gradient_grid_host(self.h_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, self.h_out,
-                                      self.ws_host)
+        self.grid_host(self.h_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, self.h_out, self.ws_host,
+                       mixed=self.mixed)
 
 
 def timed(torch, lt, fn, steps, warmup, flush, barrier):
@@ -264,7 +292,7 @@ def run_ours(args, W):
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         from paper_1902_03252_b200 import workloads
-        W = workloads.make(args.config, paper_regime=args.paper_regime, seed_offset=rank)   # own catalogue per rank
+        W = make_workload(args, seed_offset=rank)                                           # own catalogue per rank
 
     def barrier():
         if dist is not None:
@@ -310,19 +338,21 @@ def run_ours(args, W):
         # mixed: the dominant kernel is the fp64 recompute, which processes the flagged pixels only
         units = units * flagged
         peak = 2.0 * sms * LANES[mode] * sm_max * 1e6 / 1e12
-        ach = F_NOM * units / (ms_k * 1e-3) / 1e12
+        ach = r.f_nom * units / (ms_k * 1e-3) / 1e12
         return {"bound": "alu", "kernel": KERNEL_NAME[mode], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES[mode],
                 "peak_source": "derived: 2 x %d SMs x %d lanes x %.0f MHz (DESIGN.md section 8); no FP%s vector peak in "
                                "MEASURED_PEAKS.json (%s)" % (sms, LANES[mode], sm_max, "64" if LANES[mode] == 64 else "32",
                                                              peak_src),
-                "flops_per_interaction_nominal": F_NOM, "duration_ms": ms_k,
+                "flops_per_interaction_nominal": r.f_nom, "duration_ms": ms_k,
                 "interactions_per_launch": units,
                 "algorithmic_bytes_per_launch": r.out.numel() * r.out.element_size()}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": DTYPE[args.mode], "data": "synthetic",
+            "vs_baseline": (value / PAPER_V100_SIE[args.mode] if (args.model == "sie" and world == 1 and
+                                                                  args.mode in PAPER_V100_SIE) else None),
+            "dtype": DTYPE[args.mode], "data": "synthetic",
             "config": {"workload": W.name, "n_lens": int(len(W.lenses)), "nx": W.nx, "ny": W.ny, "seed": W.seed,
                        "mode": args.mode, "parallelism": "dp%d (independent catalogues, no exchange)" % world,
                        "l2": "256 MiB buffer overwritten between timed steps", "inputs": "resident in HBM"},
@@ -365,12 +395,19 @@ def run_ours(args, W):
         dist.destroy_process_group()
 
 
+def make_workload(args, seed_offset=0):
+    from paper_1902_03252_b200 import workloads
+    if args.model == "sie":
+        return workloads.make_sie("paper", seed_offset=seed_offset)
+    return workloads.make(args.config, paper_regime=args.paper_regime, seed_offset=seed_offset)
+
+
 def main():
     args = parse_args()
     if args.warmup < 3:
         args.warmup = 3
     from paper_1902_03252_b200 import workloads
-    W = workloads.make(args.config, paper_regime=args.paper_regime)
+    W = make_workload(args)
     if args.impl == "reference":
         run_reference(args, W)
     else:

@@ -48,6 +48,13 @@ typedef struct {              /* one dPIE lens; fp64; lengths in arcsec, angle i
   double b0;                  /* deflection scale (eq. 22 P:183 for its SIS meaning)                              */
 } lt_lens;
 
+typedef struct {              /* one SIE lens: the paper's own body, Algorithm 1; fp64                */
+  double x, y;                /* centre theta_center (Alg. 1 Require)                                      */
+  double epsilon;             /* pseudo-ellipticity of the potential, eq. 17-18; |epsilon| < 1        */
+  double angle;               /* Phi: counter-clockwise angle from the theta_1 axis to the semi-major axis */
+  double b0;                  /* eq. 22, arcsec                                                           */
+} lt_sie_lens;
+
 typedef enum { LT_FP64 = 0, LT_FP32 = 1, LT_MIXED = 2 } lt_precision;
 
 typedef enum {
@@ -99,6 +106,26 @@ int lt_gradient_grid(const lt_lens* d_lenses, int n_lens,
                      double x_min, double y_min, double dx, int nx, int ny,
                      lt_precision mode, const lt_mixed_params* mixed_or_null,
                      void* d_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * The same hot path with the paper's own lens body, the SIE of Algorithm 1: per lens
+ *   x' = D1 cos Phi + D2 sin Phi, y' = D2 cos Phi - D1 sin Phi (l.5-6), R = sqrt(x'^2 (1-eps) + y'^2 (1+eps)) (l.7),
+ *   g = b0 ((1-eps) x', (1+eps) y') / R (l.8-9, eq. 21), rotated back by -Phi (l.10-11) and summed (l.13-14).
+ * A pixel exactly on a lens centre (R = 0) receives nothing from that lens (reading R5).  Arguments, modes, output
+ * layout, workspace (lt_workspace_bytes / lt_host_workspace_bytes of the same sizes serve both lens models), status
+ * and mixed-rule calls exactly as for lt_gradient_grid; the mixed rule's constants are the paper's own at dx = 0.03".
+ * Domain: |epsilon| < 1, everything finite (checked on the device like the dPIE parameters).
+ */
+int lt_gradient_grid_sie(const lt_sie_lens* d_lenses, int n_lens,
+                         double x_min, double y_min, double dx, int nx, int ny,
+                         lt_precision mode, const lt_mixed_params* mixed_or_null,
+                         void* d_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+int lt_gradient_points_sie(const lt_sie_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
+                           double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+int lt_gradient_grid_sie_host(const lt_sie_lens* h_lenses, int n_lens,
+                              double x_min, double y_min, double dx, int nx, int ny,
+                              lt_precision mode, const lt_mixed_params* mixed_or_null,
+                              void* h_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
  * Gradient at an arbitrary list of points (the a9 kernel exposed; used for sampled parity at full size and for

@@ -11,6 +11,10 @@
 #include "lt_mixed.cuh"
 
 static_assert(sizeof(lt_lens) == sizeof(LtRawLens), "lt_lens and LtRawLens must have the same layout");
+static_assert(sizeof(lt_sie_lens) == sizeof(LtRawSie), "lt_sie_lens and LtRawSie must have the same layout");
+static_assert(sizeof(LtSieLens<double>) == 80 && sizeof(LtSieLens<float>) == 48, "SIE record sizes");
+template <class M> struct Rec64 { typedef typename M::template Rec<double>::type type; };
+template <class M> struct Rec32 { typedef typename M::template Rec<float>::type type; };
 static_assert(sizeof(LtLens<double>) == 128 && sizeof(LtLens<float>) == 64, "lens record sizes");
 
 namespace {
@@ -34,7 +38,7 @@ struct Layout {   // byte offsets into the workspace
   size_t header, tab64, tab32, lens64, lens32, flags, sp, list, total;
 };
 
-Layout make_layout(int n_lens, long long n_pix, bool mixed) {
+Layout make_layout(int n_lens, long long n_pix, bool mixed) {   // dPIE record sizes (the larger) serve both models
   Layout L;
   size_t o = 0;
   L.header = o; o += sizeof(LtWsHeader);
@@ -195,23 +199,24 @@ int launch_waves(int ppt, const GridArgs& a, Fn fn) {
   }
 }
 
-template <int PPT, int MINB>
-int launch_f64_ppt(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
+template <class M, int PPT, int MINB>
+int launch_f64_ppt(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
                    const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end, long long* resident) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
-                               sizeof(LtLens<double>), d);
-  const size_t smem = (size_t)chunk * sizeof(LtLens<double>);
-  if (resident) return resident_ctas(lt_grad_f64_kernel<PPT, MINB>, smem, d, *resident);
+                               sizeof(typename Rec64<M>::type), d);
+  const size_t smem = (size_t)chunk * sizeof(typename Rec64<M>::type);
+  if (resident) return resident_ctas(lt_grad_f64_kernel<M, PPT, MINB>, smem, d, *resident);
   int grid = 1;
-  const int rc = grid_for(lt_grad_f64_kernel<PPT, MINB>, smem, end - begin, d, grid);
+  const int rc = grid_for(lt_grad_f64_kernel<M, PPT, MINB>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  lt_grad_f64_kernel<PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
+  lt_grad_f64_kernel<M, PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
                                                                a.ny, tiles_x, (int)begin, (int)end, out);
   LT_CUDA(cudaGetLastError());
   ++g_launches;
   return LT_OK;
 }
-int launch_f64(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
+template <class M>
+int launch_f64(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
                const DeviceInfo& d, cudaStream_t st) {
   // 4 pixels per thread (4 independent chains, lens record loaded once per 4 interactions) at <= 128 registers, two
   // CTAs per SM; fewer pixels per thread for the ragged rest and for grids too small to give every SM two tiles
@@ -219,31 +224,34 @@ int launch_f64(const LtLens<double>* l64, const LtTables<double>* t64, const Gri
   return launch_waves(pick_ppt(g_tuning.ppt64, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
                         switch (ppt) {
-                          case 1: return launch_f64_ppt<1, 4>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
-                          case 2: return launch_f64_ppt<2, 3>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
-                          default: return launch_f64_ppt<4, 2>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                          case 1: return launch_f64_ppt<M, 1, 4>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                          case 2: return launch_f64_ppt<M, 2, 3>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                          default: return launch_f64_ppt<M, 4, 2>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
                         }
                       });
 }
 
-template <int PPT, int MINB>
-int launch_f32_ppt(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32, const GridArgs& a,
+template <class M, int PPT, int MINB>
+int launch_f32_ppt(const typename Rec64<M>::type* l64, const typename Rec32<M>::type* l32, const LtTables<float>* t32,
+                   const GridArgs& a,
                    float2* out, const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end,
                    long long* resident) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
-                               sizeof(LtLens<float>), d);
-  const size_t smem = (size_t)chunk * sizeof(LtLens<float>);
-  if (resident) return resident_ctas(lt_grad_f32_kernel<PPT, MINB>, smem, d, *resident);
+                               sizeof(typename Rec32<M>::type), d);
+  const size_t smem = (size_t)chunk * sizeof(typename Rec32<M>::type);
+  if (resident) return resident_ctas(lt_grad_f32_kernel<M, PPT, MINB>, smem, d, *resident);
   int grid = 1;
-  const int rc = grid_for(lt_grad_f32_kernel<PPT, MINB>, smem, end - begin, d, grid);
+  const int rc = grid_for(lt_grad_f32_kernel<M, PPT, MINB>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  lt_grad_f32_kernel<PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
+  lt_grad_f32_kernel<M, PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
                                                          a.ny, tiles_x, (int)begin, (int)end, out);
   LT_CUDA(cudaGetLastError());
   ++g_launches;
   return LT_OK;
 }
-int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const LtTables<float>* t32, const GridArgs& a,
+template <class M>
+int launch_f32(const typename Rec64<M>::type* l64, const typename Rec32<M>::type* l32, const LtTables<float>* t32,
+               const GridArgs& a,
                float2* out, const DeviceInfo& d, cudaStream_t st, bool hook = true) {
   // 4 pixels per thread at <= 80 registers (3 CTAs per SM): with a tighter register budget the compiler reloads the
   // constants inside the loop and the kernel, which is bound by issue slots, loses 10 %
@@ -251,25 +259,25 @@ int launch_f32(const LtLens<double>* l64, const LtLens<float>* l32, const LtTabl
   return launch_waves(pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
                         switch (ppt) {
-                          case 1: return launch_f32_ppt<1, 6>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
-                          case 2: return launch_f32_ppt<2, 4>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
-                          default: return launch_f32_ppt<4, 3>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          case 1: return launch_f32_ppt<M, 1, 6>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          case 2: return launch_f32_ppt<M, 2, 4>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          default: return launch_f32_ppt<M, 4, 3>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
                         }
                       });
 }
 
-template <bool FROM_LIST>
-int launch_list(const LtLens<double>* l64, const LtTables<double>* t64, const GridArgs& a, const unsigned int* list, const LtWsHeader* hdr,
+template <class M, bool FROM_LIST>
+int launch_list(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, const unsigned int* list, const LtWsHeader* hdr,
                 const double2* points, long long n_points, long long max_work, double2* out, const DeviceInfo& d,
                 cudaStream_t st) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
-                               sizeof(LtLens<double>), d);
-  const size_t smem = (size_t)chunk * sizeof(LtLens<double>);
+                               sizeof(typename Rec64<M>::type), d);
+  const size_t smem = (size_t)chunk * sizeof(typename Rec64<M>::type);
   int grid = 1;
-  const int rc = grid_for(lt_grad_list_f64_kernel<FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
+  const int rc = grid_for(lt_grad_list_f64_kernel<M, FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
   if (rc != LT_OK) return rc;
   KernelEvents ke(st, FROM_LIST);
-  lt_grad_list_f64_kernel<FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
+  lt_grad_list_f64_kernel<M, FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
                                                                     a.nx, list, hdr, points, n_points, out);
   LT_CUDA(cudaGetLastError());
   ++g_launches;
@@ -284,12 +292,13 @@ int check_mixed(const lt_mixed_params& m) {
   return ok ? LT_OK : LT_ERR_BAD_MIXED_PARAMS;
 }
 
-int precompute(const lt_lens* d_lenses, int n_lens, double dx, unsigned char* ws, const Layout& L, cudaStream_t st) {
+template <class M>
+int precompute(const void* d_lenses, int n_lens, double dx, unsigned char* ws, const Layout& L, cudaStream_t st) {
   LT_CUDA(cudaMemsetAsync(ws + L.header, 0, sizeof(LtWsHeader), st));
   const int blocks = n_lens > 0 ? (n_lens + 127) / 128 : 1;
-  lt_precompute_kernel<<<blocks, 128, 0, st>>>(reinterpret_cast<const LtRawLens*>(d_lenses), n_lens, dx,
-                                               reinterpret_cast<LtLens<double>*>(ws + L.lens64),
-                                               reinterpret_cast<LtLens<float>*>(ws + L.lens32),
+  lt_precompute_kernel<M><<<blocks, 128, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, dx,
+                                               reinterpret_cast<typename Rec64<M>::type*>(ws + L.lens64),
+                                               reinterpret_cast<typename Rec32<M>::type*>(ws + L.lens32),
                                                reinterpret_cast<LtTables<double>*>(ws + L.tab64),
                                                reinterpret_cast<LtTables<float>*>(ws + L.tab32),
                                                reinterpret_cast<LtWsHeader*>(ws + L.header));
@@ -320,6 +329,126 @@ __global__ void __launch_bounds__(256) lt_probe_kernel(int iters, T seed) {
     if (sizeof(T) == 8) lt_probe_sink64 = (double)s; else lt_probe_sink32 = (float)s;
   }
 }
+
+// ------------------------------------------------------------------------------------------------ entry points, per lens model
+namespace {
+
+template <class M>
+int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                     lt_precision mode, const lt_mixed_params* mixed_or_null, void* d_out_grad, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream) {
+  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
+  if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return LT_ERR_BAD_MODE;
+  if (!d_out_grad || !d_workspace || (n_lens > 0 && !d_lenses)) return LT_ERR_NULL_POINTER;
+  if (!(isfinite(x_min) && isfinite(y_min) && isfinite(dx)) || !(dx > 0.0)) return LT_ERR_BAD_GRID;
+  if (((uintptr_t)d_out_grad & 15) || ((uintptr_t)d_workspace & 15)) return LT_ERR_MISALIGNED;
+  const long long n_pix = (long long)nx * ny;
+  const Layout L = make_layout(n_lens, n_pix, mode == LT_MIXED);
+  if (workspace_bytes < L.total) return LT_ERR_WORKSPACE_TOO_SMALL;
+  lt_mixed_params mp;
+  lt_mixed_defaults(&mp);
+  if (mode == LT_MIXED && mixed_or_null) {
+    mp = *mixed_or_null;
+    const int rc = check_mixed(mp);
+    if (rc != LT_OK) return rc;
+  }
+  DeviceInfo dev;
+  int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)d_workspace;
+  LtWsHeader* hdr = reinterpret_cast<LtWsHeader*>(ws + L.header);
+  const typename Rec64<M>::type* l64 = reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64);
+  const typename Rec32<M>::type* l32 = reinterpret_cast<const typename Rec32<M>::type*>(ws + L.lens32);
+  const LtTables<double>* t64 = reinterpret_cast<const LtTables<double>*>(ws + L.tab64);
+  const LtTables<float>* t32 = reinterpret_cast<const LtTables<float>*>(ws + L.tab32);
+  const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
+
+  rc = precompute<M>(d_lenses, n_lens, dx, ws, L, st);                                   /* a1 */
+  if (rc != LT_OK) return rc;
+  if (mode == LT_FP64) return launch_f64<M>(l64, t64, a, (double2*)d_out_grad, dev, st);      /* a2-a7 */
+  if (mode == LT_FP32) return launch_f32<M>(l64, l32, t32, a, (float2*)d_out_grad, dev, st);
+
+  /* LT_MIXED (P:330): single precision everywhere, flag, double precision on the flagged pixels */
+  unsigned char* flags = ws + L.flags;
+  float2* sp = reinterpret_cast<float2*>(ws + L.sp);
+  unsigned int* list = reinterpret_cast<unsigned int*>(ws + L.list);
+  LtMixedDev md;
+  md.fdx = (float)dx;
+  md.t25 = (float)(dx / mp.m_max);
+  md.t28 = (float)(mp.c28 * dx);
+  md.h_cluster = mp.patch_halfwidth_cluster;
+  md.h_galaxy = mp.patch_halfwidth_galaxy;
+  md.b0_cluster = mp.b0_cluster_threshold;
+  LT_CUDA(cudaMemsetAsync(flags, 0, (size_t)n_pix, st));
+  if (n_lens > 0) {
+    lt_patch_kernel<typename M::Raw><<<n_lens, 256, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, x_min, y_min, dx,
+                                            nx, ny, md, flags);
+    LT_CUDA(cudaGetLastError());
+    ++g_launches;
+  }
+  rc = launch_f32<M>(l64, l32, t32, a, sp, dev, st, /*hook=*/false);
+  if (rc != LT_OK) return rc;
+  {
+    long long blocks = (n_pix + 255) / 256;
+    const long long cap = (long long)dev.sms * 16;
+    if (blocks > cap) blocks = cap;
+    lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, (double2*)d_out_grad, list, hdr);   /* a8 */
+    LT_CUDA(cudaGetLastError());
+    ++g_launches;
+  }
+  return launch_list<M, true>(l64, t64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
+}
+
+template <class M>
+int gradient_points_impl(const void* d_lenses, int n_lens, const double* d_points, long long n_points,
+                       double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!sizes_ok(n_lens, 1, 1) || n_points < 0) return LT_ERR_BAD_SIZE;
+  if (!d_workspace || (n_lens > 0 && !d_lenses) || (n_points > 0 && (!d_points || !d_out))) return LT_ERR_NULL_POINTER;
+  if (((uintptr_t)d_out & 15) || ((uintptr_t)d_points & 15) || ((uintptr_t)d_workspace & 15)) return LT_ERR_MISALIGNED;
+  const Layout L = make_layout(n_lens, 1, false);
+  if (workspace_bytes < L.total) return LT_ERR_WORKSPACE_TOO_SMALL;
+  DeviceInfo dev;
+  int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)d_workspace;
+  rc = precompute<M>(d_lenses, n_lens, 1.0, ws, L, st);
+  if (rc != LT_OK || n_points == 0) return rc;
+  const GridArgs a{n_lens, 0.0, 0.0, 1.0, 1, 1};
+  return launch_list<M, false>(reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
+                            reinterpret_cast<const LtTables<double>*>(ws + L.tab64), a, nullptr,
+                            reinterpret_cast<const LtWsHeader*>(ws + L.header),
+                            reinterpret_cast<const double2*>(d_points), n_points, n_points,
+                            reinterpret_cast<double2*>(d_out), dev, st);
+}
+
+template <class M>
+int gradient_grid_host_impl(const void* h_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                          lt_precision mode, const lt_mixed_params* mixed_or_null, void* h_out_grad,
+                          void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
+  if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return LT_ERR_BAD_MODE;
+  if (!h_out_grad || !d_workspace || (n_lens > 0 && !h_lenses)) return LT_ERR_NULL_POINTER;
+  if ((uintptr_t)d_workspace & 15) return LT_ERR_MISALIGNED;
+  if (workspace_bytes < lt_host_workspace_bytes(n_lens, nx, ny, mode)) return LT_ERR_WORKSPACE_TOO_SMALL;
+  const size_t w = align_up(lt_workspace_bytes(n_lens, nx, ny, mode));
+  const size_t lens_bytes = (size_t)n_lens * sizeof(typename M::Raw);
+  const size_t elem = (mode == LT_FP32) ? sizeof(float2) : sizeof(double2);
+  unsigned char* ws = (unsigned char*)d_workspace;
+  void* d_lenses = ws + w;
+  void* d_out = ws + w + align_up(lens_bytes);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (n_lens > 0) LT_CUDA(cudaMemcpyAsync(d_lenses, h_lenses, lens_bytes, cudaMemcpyHostToDevice, st));
+  const int rc = gradient_grid_impl<M>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out, ws, w, st);
+  if (rc != LT_OK) return rc;
+  LT_CUDA(cudaMemcpyAsync(h_out_grad, d_out, (size_t)nx * ny * elem, cudaMemcpyDeviceToHost, st));
+  return LT_OK;
+}
+
+}  // namespace
 
 // ------------------------------------------------------------------------------------------------ C ABI
 extern "C" {
@@ -379,96 +508,6 @@ size_t lt_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode) {
   return make_layout(n_lens, (long long)nx * ny, mode == LT_MIXED).total;
 }
 
-int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
-                     lt_precision mode, const lt_mixed_params* mixed_or_null, void* d_out_grad, void* d_workspace,
-                     size_t workspace_bytes, void* cuda_stream) {
-  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
-  if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return LT_ERR_BAD_MODE;
-  if (!d_out_grad || !d_workspace || (n_lens > 0 && !d_lenses)) return LT_ERR_NULL_POINTER;
-  if (!(isfinite(x_min) && isfinite(y_min) && isfinite(dx)) || !(dx > 0.0)) return LT_ERR_BAD_GRID;
-  if (((uintptr_t)d_out_grad & 15) || ((uintptr_t)d_workspace & 15)) return LT_ERR_MISALIGNED;
-  const long long n_pix = (long long)nx * ny;
-  const Layout L = make_layout(n_lens, n_pix, mode == LT_MIXED);
-  if (workspace_bytes < L.total) return LT_ERR_WORKSPACE_TOO_SMALL;
-  lt_mixed_params mp;
-  lt_mixed_defaults(&mp);
-  if (mode == LT_MIXED && mixed_or_null) {
-    mp = *mixed_or_null;
-    const int rc = check_mixed(mp);
-    if (rc != LT_OK) return rc;
-  }
-  DeviceInfo dev;
-  int rc = device_info(dev);
-  if (rc != LT_OK) return rc;
-  g_launches = 0;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  unsigned char* ws = (unsigned char*)d_workspace;
-  LtWsHeader* hdr = reinterpret_cast<LtWsHeader*>(ws + L.header);
-  const LtLens<double>* l64 = reinterpret_cast<const LtLens<double>*>(ws + L.lens64);
-  const LtLens<float>* l32 = reinterpret_cast<const LtLens<float>*>(ws + L.lens32);
-  const LtTables<double>* t64 = reinterpret_cast<const LtTables<double>*>(ws + L.tab64);
-  const LtTables<float>* t32 = reinterpret_cast<const LtTables<float>*>(ws + L.tab32);
-  const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
-
-  rc = precompute(d_lenses, n_lens, dx, ws, L, st);                                   /* a1 */
-  if (rc != LT_OK) return rc;
-  if (mode == LT_FP64) return launch_f64(l64, t64, a, (double2*)d_out_grad, dev, st);      /* a2-a7 */
-  if (mode == LT_FP32) return launch_f32(l64, l32, t32, a, (float2*)d_out_grad, dev, st);
-
-  /* LT_MIXED (P:330): single precision everywhere, flag, double precision on the flagged pixels */
-  unsigned char* flags = ws + L.flags;
-  float2* sp = reinterpret_cast<float2*>(ws + L.sp);
-  unsigned int* list = reinterpret_cast<unsigned int*>(ws + L.list);
-  LtMixedDev md;
-  md.fdx = (float)dx;
-  md.t25 = (float)(dx / mp.m_max);
-  md.t28 = (float)(mp.c28 * dx);
-  md.h_cluster = mp.patch_halfwidth_cluster;
-  md.h_galaxy = mp.patch_halfwidth_galaxy;
-  md.b0_cluster = mp.b0_cluster_threshold;
-  LT_CUDA(cudaMemsetAsync(flags, 0, (size_t)n_pix, st));
-  if (n_lens > 0) {
-    lt_patch_kernel<<<n_lens, 256, 0, st>>>(reinterpret_cast<const LtRawLens*>(d_lenses), n_lens, x_min, y_min, dx,
-                                            nx, ny, md, flags);
-    LT_CUDA(cudaGetLastError());
-    ++g_launches;
-  }
-  rc = launch_f32(l64, l32, t32, a, sp, dev, st, /*hook=*/false);
-  if (rc != LT_OK) return rc;
-  {
-    long long blocks = (n_pix + 255) / 256;
-    const long long cap = (long long)dev.sms * 16;
-    if (blocks > cap) blocks = cap;
-    lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, (double2*)d_out_grad, list, hdr);   /* a8 */
-    LT_CUDA(cudaGetLastError());
-    ++g_launches;
-  }
-  return launch_list<true>(l64, t64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
-}
-
-int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
-                       double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
-  if (!sizes_ok(n_lens, 1, 1) || n_points < 0) return LT_ERR_BAD_SIZE;
-  if (!d_workspace || (n_lens > 0 && !d_lenses) || (n_points > 0 && (!d_points || !d_out))) return LT_ERR_NULL_POINTER;
-  if (((uintptr_t)d_out & 15) || ((uintptr_t)d_points & 15) || ((uintptr_t)d_workspace & 15)) return LT_ERR_MISALIGNED;
-  const Layout L = make_layout(n_lens, 1, false);
-  if (workspace_bytes < L.total) return LT_ERR_WORKSPACE_TOO_SMALL;
-  DeviceInfo dev;
-  int rc = device_info(dev);
-  if (rc != LT_OK) return rc;
-  g_launches = 0;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  unsigned char* ws = (unsigned char*)d_workspace;
-  rc = precompute(d_lenses, n_lens, 1.0, ws, L, st);
-  if (rc != LT_OK || n_points == 0) return rc;
-  const GridArgs a{n_lens, 0.0, 0.0, 1.0, 1, 1};
-  return launch_list<false>(reinterpret_cast<const LtLens<double>*>(ws + L.lens64),
-                            reinterpret_cast<const LtTables<double>*>(ws + L.tab64), a, nullptr,
-                            reinterpret_cast<const LtWsHeader*>(ws + L.header),
-                            reinterpret_cast<const double2*>(d_points), n_points, n_points,
-                            reinterpret_cast<double2*>(d_out), dev, st);
-}
-
 size_t lt_host_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode) {
   const size_t w = lt_workspace_bytes(n_lens, nx, ny, mode);
   if (w == 0) return 0;
@@ -476,26 +515,41 @@ size_t lt_host_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode) {
   return align_up(w) + align_up((size_t)n_lens * sizeof(lt_lens)) + align_up((size_t)nx * ny * elem);
 }
 
+int lt_gradient_grid(const lt_lens* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                     lt_precision mode, const lt_mixed_params* mixed_or_null, void* d_out_grad, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream) {
+  return gradient_grid_impl<LtDpieModel>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out_grad,
+                                         d_workspace, workspace_bytes, cuda_stream);
+}
+int lt_gradient_grid_sie(const lt_sie_lens* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                         lt_precision mode, const lt_mixed_params* mixed_or_null, void* d_out_grad, void* d_workspace,
+                         size_t workspace_bytes, void* cuda_stream) {
+  return gradient_grid_impl<LtSieModel>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out_grad,
+                                        d_workspace, workspace_bytes, cuda_stream);
+}
+
+int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
+                       double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  return gradient_points_impl<LtDpieModel>(d_lenses, n_lens, d_points, n_points, d_out, d_workspace, workspace_bytes,
+                                           cuda_stream);
+}
+int lt_gradient_points_sie(const lt_sie_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
+                           double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  return gradient_points_impl<LtSieModel>(d_lenses, n_lens, d_points, n_points, d_out, d_workspace, workspace_bytes,
+                                          cuda_stream);
+}
+
 int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
                           lt_precision mode, const lt_mixed_params* mixed_or_null, void* h_out_grad,
                           void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
-  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
-  if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return LT_ERR_BAD_MODE;
-  if (!h_out_grad || !d_workspace || (n_lens > 0 && !h_lenses)) return LT_ERR_NULL_POINTER;
-  if ((uintptr_t)d_workspace & 15) return LT_ERR_MISALIGNED;
-  if (workspace_bytes < lt_host_workspace_bytes(n_lens, nx, ny, mode)) return LT_ERR_WORKSPACE_TOO_SMALL;
-  const size_t w = align_up(lt_workspace_bytes(n_lens, nx, ny, mode));
-  const size_t lens_bytes = (size_t)n_lens * sizeof(lt_lens);
-  const size_t elem = (mode == LT_FP32) ? sizeof(float2) : sizeof(double2);
-  unsigned char* ws = (unsigned char*)d_workspace;
-  lt_lens* d_lenses = reinterpret_cast<lt_lens*>(ws + w);
-  void* d_out = ws + w + align_up(lens_bytes);
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (n_lens > 0) LT_CUDA(cudaMemcpyAsync(d_lenses, h_lenses, lens_bytes, cudaMemcpyHostToDevice, st));
-  const int rc = lt_gradient_grid(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out, ws, w, st);
-  if (rc != LT_OK) return rc;
-  LT_CUDA(cudaMemcpyAsync(h_out_grad, d_out, (size_t)nx * ny * elem, cudaMemcpyDeviceToHost, st));
-  return LT_OK;
+  return gradient_grid_host_impl<LtDpieModel>(h_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
+                                              h_out_grad, d_workspace, workspace_bytes, cuda_stream);
+}
+int lt_gradient_grid_sie_host(const lt_sie_lens* h_lenses, int n_lens, double x_min, double y_min, double dx, int nx,
+                              int ny, lt_precision mode, const lt_mixed_params* mixed_or_null, void* h_out_grad,
+                              void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  return gradient_grid_host_impl<LtSieModel>(h_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
+                                             h_out_grad, d_workspace, workspace_bytes, cuda_stream);
 }
 
 int lt_last_status(const void* d_workspace, void* cuda_stream, int* bad_lens_or_null) {

@@ -28,25 +28,27 @@ struct LtWsHeader {                 // first 256 bytes of the workspace; zeroed 
 static_assert(sizeof(LtWsHeader) == 256, "workspace header is 256 bytes");
 
 // ------------------------------------------------------------------------------------------------ a1: precompute
-__global__ void lt_precompute_kernel(const LtRawLens* __restrict__ raw, int n_lens, double dx,
-                                     LtLens<double>* __restrict__ l64, LtLens<float>* __restrict__ l32,
+template <class M>
+__global__ void lt_precompute_kernel(const typename M::Raw* __restrict__ raw, int n_lens, double dx,
+                                     typename M::template Rec<double>::type* __restrict__ l64,
+                                     typename M::template Rec<float>::type* __restrict__ l32,
                                      LtTables<double>* __restrict__ t64, LtTables<float>* __restrict__ t32,
                                      LtWsHeader* __restrict__ hdr) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k == 0) hdr->n_lens = n_lens;
-  if (blockIdx.x == gridDim.x - 1)           // the last block also writes the range-reduction tables (lt_math.cuh)
+  if (M::kTables && blockIdx.x == gridDim.x - 1)   // the last block also writes the range-reduction tables (lt_math.cuh)
     for (int e = threadIdx.x; e < LT_TABLE_ENTRIES; e += blockDim.x) lt_fill_table_entry(e, *t64, *t32);
   if (k >= n_lens) return;
-  const LtRawLens r = raw[k];
-  LtLens<double> D;
-  if (lt_lens_valid(r)) {
-    lt_pack_lens(r, D);
+  const typename M::Raw r = raw[k];
+  typename M::template Rec<double>::type D;
+  if (M::valid(r)) {
+    M::pack(r, D);
   } else {
-    lt_poison_lens(D);
+    M::poison(D);
     atomicMax(&hdr->bad_code, n_lens - k);
   }
-  LtLens<float> F;
-  lt_round_lens(D, dx, F);
+  typename M::template Rec<float>::type F;
+  M::round(D, dx, F);
   l64[k] = D;
   l32[k] = F;
 }
@@ -58,24 +60,37 @@ __device__ __forceinline__ void lt_copy16(void* dst, const void* src, int count)
   for (int w = threadIdx.x; w < count; w += blockDim.x) d[w] = s[w];
 }
 
+// One interaction of lens model M given the sky-frame offset d1 = theta_1 - xc and the two per-row products
+// d2sx = d2 * sx, d2cy = d2 * cy (d2 = theta_2 - yc; shared by the pixels of a row): a3 (rotate, scaled: Alg. 1 l.5-6
+// with the model's factors folded into cos/sin), then the model's body and back rotation (a4-a6).
+template <class M, class T, class R>
+__device__ __forceinline__ void lt_model_interaction(const T d1, const T d2sx, const T d2cy, const R& L,
+                                                     const LtTables<T>& tab, T& G1, T& G2) {
+  const T X = lt_fma(d1, L.cx, d2sx);
+  const T Y = lt_fma(-d1, L.sy, d2cy);
+  M::template interact<T>(X, Y, L, tab, G1, G2);
+}
+
 // ------------------------------------------------------------------------------------------------ fp64 grid kernel
 // a2 pixel coordinate (x_min + i*dx, product and sum rounded separately, exactly as the API states it), a3-a6 per
 // lens (lt_interaction), a7 one double2 store per pixel.
-template <int PPT, int MINB>
+template <class M, int PPT, int MINB>
 __global__ void __launch_bounds__(LT_THREADS, MINB)
-lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<double>* __restrict__ tables, int n_lens,
+lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ lens,
+                   const LtTables<double>* __restrict__ tables, int n_lens,
                    int chunk, double x_min, double y_min, double dx, int nx, int ny, int tiles_x, int tile_begin,
                    int tile_end, double2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
+  typedef typename M::template Rec<double>::type Rec;
   __shared__ LtTables<double> tab;
-  LtLens<double>* sl = reinterpret_cast<LtLens<double>*>(lt_smem);
-  lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
   __syncthreads();
   constexpr int TILE_W = 32 * PPT;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   const bool single = n_lens <= chunk;
   if (single) {
-    lt_copy16(sl, lens, n_lens * (int)(sizeof(LtLens<double>) / 16));
+    lt_copy16(sl, lens, n_lens * (int)(sizeof(Rec) / 16));
     __syncthreads();
   }
   for (int tile = tile_begin + blockIdx.x; tile < tile_end; tile += gridDim.x) {
@@ -94,16 +109,16 @@ lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<doubl
       const int cnt = min(chunk, n_lens - base);
       if (!single) {
         __syncthreads();
-        lt_copy16(sl, lens + base, cnt * (int)(sizeof(LtLens<double>) / 16));
+        lt_copy16(sl, lens + base, cnt * (int)(sizeof(Rec) / 16));
         __syncthreads();
       }
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
-        const LtLens<double> L = sl[k];
+        const Rec L = sl[k];
         const double d2 = t2 - L.y0;                                // Alg. 1 l.4
         const double d2sx = d2 * L.sx, d2cy = d2 * L.cy;
 #pragma unroll
-        for (int p = 0; p < PPT; ++p) lt_interaction<double>(t1[p] - L.x0, d2sx, d2cy, L, tab, G1[p], G2[p]);  // l.3, l.5-14
+        for (int p = 0; p < PPT; ++p) lt_model_interaction<M, double>(t1[p] - L.x0, d2sx, d2cy, L, tab, G1[p], G2[p]);  // l.3, l.5-14
       }
     }
     if (j < ny) {
@@ -123,15 +138,18 @@ lt_grad_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<doubl
 //   x' = X0 + il*(dx cos) + jl*(dx sin),  y' = Y0 + jl*(dx cos) - il*(dx sin)      (Alg. 1 l.3-6 merged)
 // so the fp32 rounding of the coordinate is relative to the tile size, not to |theta| (the |theta_c|/|dtheta| term of
 // (A.65)).  All per-interaction arithmetic is FP32.
-template <int PPT, int MINB>
+template <class M, int PPT, int MINB>
 __global__ void __launch_bounds__(LT_THREADS, MINB)
-lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float>* __restrict__ lens32,
+lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ lens64,
+                   const typename M::template Rec<float>::type* __restrict__ lens32,
                    const LtTables<float>* __restrict__ tables, int n_lens, int chunk, double x_min, double y_min,
                    double dx, int nx, int ny, int tiles_x, int tile_begin, int tile_end, float2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
+  typedef typename M::template Rec<float>::type Rec;
+  typedef typename M::template Rec<double>::type Rec64;
   __shared__ LtTables<float> tab;
-  LtLens<float>* sl = reinterpret_cast<LtLens<float>*>(lt_smem);
-  lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));   // visible after the first __syncthreads of the chunk loop
+  Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));   // visible after the first __syncthreads of the chunk loop
   constexpr int TILE_W = 32 * PPT;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   // in-tile offsets from the tile centre, in pixels (exact in fp32)
@@ -156,8 +174,8 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
       const int cnt = min(chunk, n_lens - base);
       __syncthreads();
       for (int k = threadIdx.x; k < cnt; k += LT_THREADS) {
-        LtLens<float> F = lens32[base + k];
-        const LtLens<double>& D = lens64[base + k];
+        Rec F = lens32[base + k];
+        const Rec64& D = lens64[base + k];
         const double d1 = cx - D.x0, d2 = cy - D.y0;
         F.x0 = (float)fma(d1, D.cx, d2 * D.sx);
         F.y0 = (float)fma(-d1, D.sy, d2 * D.cy);
@@ -166,16 +184,14 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
       __syncthreads();
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
-        const LtLens<float> L = sl[k];
+        const Rec L = sl[k];
         const float xr = fmaf(jl, L.sx, L.x0);
         const float yr = fmaf(jl, L.cy, L.y0);
 #pragma unroll
         for (int p = 0; p < PPT; ++p) {
           const float x = fmaf(il[p], L.cx, xr);
           const float y = fmaf(-il[p], L.sy, yr);
-          float ax, ay;
-          lt_dpie_body<float>(x, y, L, tab, ax, ay);
-          lt_accumulate<float>(ax, ay, L, G1[p], G2[p]);          // Alg. 1 l.10-11 + l.13-14
+          M::template interact<float>(x, y, L, tab, G1[p], G2[p]);   // Alg. 1 l.7-14
         }
       }
     }
@@ -196,8 +212,9 @@ lt_grad_f32_kernel(const LtLens<double>* __restrict__ lens64, const LtLens<float
 // Groups of 4 * 256 entries, 4 per thread (entries 256 apart, so list reads stay coalesced); a rest of at most one
 // 256-entry group per CTA after the whole waves runs one entry per thread (the count is only known on the device, so
 // the split is made here, not on the host).
-template <bool FROM_LIST, int PPT>
-__device__ __forceinline__ void lt_list_group(const LtLens<double>* __restrict__ lens, const LtLens<double>* sl,
+template <class M, bool FROM_LIST, int PPT>
+__device__ __forceinline__ void lt_list_group(const typename M::template Rec<double>::type* __restrict__ lens,
+                                              const typename M::template Rec<double>::type* sl,
                                               const LtTables<double>& tab, int n_lens, int chunk, bool single,
                                               double x_min, double y_min, double dx, int nx,
                                               const unsigned int* __restrict__ list,
@@ -230,16 +247,17 @@ __device__ __forceinline__ void lt_list_group(const LtLens<double>* __restrict__
     const int cnt = min(chunk, n_lens - base);
     if (!single) {
       __syncthreads();
-      lt_copy16(const_cast<LtLens<double>*>(sl), lens + base, cnt * (int)(sizeof(LtLens<double>) / 16));
+      lt_copy16(const_cast<typename M::template Rec<double>::type*>(sl), lens + base,
+                cnt * (int)(sizeof(typename M::template Rec<double>::type) / 16));
       __syncthreads();
     }
 #pragma unroll 1
     for (int k = 0; k < cnt; ++k) {
-      const LtLens<double> L = sl[k];
+      const typename M::template Rec<double>::type L = sl[k];
 #pragma unroll
       for (int p = 0; p < PPT; ++p) {
         const double d2 = t2[p] - L.y0;
-        lt_interaction<double>(t1[p] - L.x0, d2 * L.sx, d2 * L.cy, L, tab, G1[p], G2[p]);
+        lt_model_interaction<M, double>(t1[p] - L.x0, d2 * L.sx, d2 * L.cy, L, tab, G1[p], G2[p]);
       }
     }
   }
@@ -248,21 +266,22 @@ __device__ __forceinline__ void lt_list_group(const LtLens<double>* __restrict__
     if (live[p]) out[dst[p]] = make_double2(G1[p], G2[p]);
 }
 
-template <bool FROM_LIST>
+template <class M, bool FROM_LIST>
 __global__ void __launch_bounds__(LT_THREADS, 2)
-lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<double>* __restrict__ tables,
+lt_grad_list_f64_kernel(const typename M::template Rec<double>::type* __restrict__ lens, const LtTables<double>* __restrict__ tables,
                         int n_lens, int chunk, double x_min, double y_min, double dx, int nx,
                         const unsigned int* __restrict__ list, const LtWsHeader* __restrict__ hdr,
                         const double2* __restrict__ points, long long n_points, double2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
+  typedef typename M::template Rec<double>::type Rec;
   __shared__ LtTables<double> tab;
-  LtLens<double>* sl = reinterpret_cast<LtLens<double>*>(lt_smem);
-  lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
   __syncthreads();
   const long long total = FROM_LIST ? (long long)hdr->list_count : n_points;
   const bool single = n_lens <= chunk;
   if (single) {
-    lt_copy16(sl, lens, n_lens * (int)(sizeof(LtLens<double>) / 16));
+    lt_copy16(sl, lens, n_lens * (int)(sizeof(Rec) / 16));
     __syncthreads();
   }
   constexpr int WIDE = 4;
@@ -274,10 +293,10 @@ lt_grad_list_f64_kernel(const LtLens<double>* __restrict__ lens, const LtTables<
     rest0 = total;
   }
   for (long long g = blockIdx.x; g < n_wide; g += gridDim.x)
-    lt_list_group<FROM_LIST, WIDE>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
+    lt_list_group<M, FROM_LIST, WIDE>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
                                    g * (WIDE * LT_THREADS), total, out);
   const long long n_rest = (total - rest0 + LT_THREADS - 1) / LT_THREADS;   // <= gridDim.x
   for (long long g = blockIdx.x; g < n_rest; g += gridDim.x)
-    lt_list_group<FROM_LIST, 1>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
+    lt_list_group<M, FROM_LIST, 1>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
                                 rest0 + g * LT_THREADS, total, out);
 }

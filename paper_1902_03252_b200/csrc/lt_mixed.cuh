@@ -18,7 +18,8 @@ struct LtMixedDev {          // host-prepared constants of the rule
 // a8, part 1: one CTA per lens marks its DP patch: the box of half-width hp = max(1, ceil(h/dx)) pixels centred on the
 // pixel nearest the lens centre, clipped to the grid (R14); h by lens class (b0 >= threshold: cluster-scale, R15).
 // Overlapping patches write the same value, so plain stores are race-free in effect.
-__global__ void lt_patch_kernel(const LtRawLens* __restrict__ raw, int n_lens, double x_min, double y_min, double dx,
+template <class Raw>
+__global__ void lt_patch_kernel(const Raw* __restrict__ raw, int n_lens, double x_min, double y_min, double dx,
                                 int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags) {
   const int k = blockIdx.x;
   if (k >= n_lens) return;

@@ -21,6 +21,7 @@ _LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
 
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
+           "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host",
            "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
 
 
@@ -71,6 +72,11 @@ def lib():
         L.lt_gradient_grid_host.restype = ci
         L.lt_gradient_points.argtypes = [vp, ci, vp, cll, vp, vp, sz, vp]
         L.lt_gradient_points.restype = ci
+        for name in ("lt_gradient_grid_sie", "lt_gradient_grid_sie_host"):
+            getattr(L, name).argtypes = L.lt_gradient_grid.argtypes
+            getattr(L, name).restype = ci
+        L.lt_gradient_points_sie.argtypes = L.lt_gradient_points.argtypes
+        L.lt_gradient_points_sie.restype = ci
         L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci, ci]
         L.lt_last_launch_count.restype = ci
         L.lt_set_tuning.restype = ci
@@ -98,10 +104,10 @@ def _stream(stream):
     return ctypes.c_void_p(s.cuda_stream)
 
 
-def _lenses_dev(lenses):
+def _lenses_dev(lenses, cols=7):
     if not (isinstance(lenses, torch.Tensor) and lenses.is_cuda and lenses.dtype == torch.float64):
-        raise TypeError("lenses must be a CUDA float64 tensor [n_lens, 7]")
-    lenses = lenses.reshape(-1, 7)
+        raise TypeError("lenses must be a CUDA float64 tensor [n_lens, %d]" % cols)
+    lenses = lenses.reshape(-1, cols)
     if not lenses.is_contiguous():
         lenses = lenses.contiguous()
     return lenses
@@ -162,9 +168,9 @@ def alloc_workspace(n_lens, nx, ny, mode, device="cuda", host=False):
 
 
 def lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None, out=None, workspace=None,
-                     stream=None):
+                     stream=None, _fn="lt_gradient_grid", _cols=7):
     """Deflection map on the device.  Returns `out` ([ny, nx, 2]; float32 for LT_FP32, else float64).  Asynchronous."""
-    lenses = _lenses_dev(lenses)
+    lenses = _lenses_dev(lenses, _cols)
     n_lens = lenses.shape[0]
     dt = torch.float32 if mode == LT_FP32 else torch.float64
     if out is None:
@@ -173,34 +179,47 @@ def lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None,
         raise TypeError("out must be a contiguous CUDA %s tensor with nx*ny*2 elements" % dt)
     if workspace is None:
         workspace = alloc_workspace(n_lens, nx, ny, mode, lenses.device)
-    rc = lib().lt_gradient_grid(ctypes.c_void_p(lenses.data_ptr() if n_lens else None), n_lens, float(x_min),
-                                float(y_min), float(dx), int(nx), int(ny), int(mode), _mixed_ptr(mixed),
-                                ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
-                                workspace.numel(), _stream(stream))
-    _check(rc, "lt_gradient_grid")
+    rc = getattr(lib(), _fn)(ctypes.c_void_p(lenses.data_ptr() if n_lens else None), n_lens, float(x_min),
+                             float(y_min), float(dx), int(nx), int(ny), int(mode), _mixed_ptr(mixed),
+                             ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
+                             workspace.numel(), _stream(stream))
+    _check(rc, _fn)
     return out
 
 
-def lt_gradient_grid_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, workspace, mixed=None, stream=None):
+def lt_gradient_grid_sie(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None, out=None, workspace=None,
+                         stream=None):
+    """The same with the paper's SIE body (Algorithm 1); lenses: CUDA float64 [n_lens, 5] = (xc, yc, eps, Phi, b0)."""
+    return lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode, mixed, out, workspace, stream,
+                            _fn="lt_gradient_grid_sie", _cols=5)
+
+
+def lt_gradient_grid_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, workspace, mixed=None, stream=None,
+                          _fn="lt_gradient_grid_host", _cols=7):
     """End-to-end call with HOST buffers (CPU tensors, ideally pinned): H2D of the catalogue, the hot path, D2H of the
     map, all enqueued on the stream.  The caller synchronises before reading h_out."""
     if h_lenses.is_cuda or h_out.is_cuda or h_lenses.dtype != torch.float64 or not h_lenses.is_contiguous():
         raise TypeError("h_lenses / h_out must be contiguous CPU tensors (float64 catalogue)")
-    n_lens = h_lenses.reshape(-1, 7).shape[0]
+    n_lens = h_lenses.reshape(-1, _cols).shape[0]
     dt = torch.float32 if mode == LT_FP32 else torch.float64
     if h_out.dtype != dt or h_out.numel() != nx * ny * 2 or not h_out.is_contiguous():
         raise TypeError("h_out must be a contiguous CPU %s tensor with nx*ny*2 elements" % dt)
-    rc = lib().lt_gradient_grid_host(ctypes.c_void_p(h_lenses.data_ptr() if n_lens else None), n_lens, float(x_min),
-                                     float(y_min), float(dx), int(nx), int(ny), int(mode), _mixed_ptr(mixed),
-                                     ctypes.c_void_p(h_out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
-                                     workspace.numel(), _stream(stream))
-    _check(rc, "lt_gradient_grid_host")
+    rc = getattr(lib(), _fn)(ctypes.c_void_p(h_lenses.data_ptr() if n_lens else None), n_lens, float(x_min),
+                             float(y_min), float(dx), int(nx), int(ny), int(mode), _mixed_ptr(mixed),
+                             ctypes.c_void_p(h_out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
+                             workspace.numel(), _stream(stream))
+    _check(rc, _fn)
     return h_out
 
 
-def lt_gradient_points(lenses, points, out=None, workspace=None, stream=None):
+def lt_gradient_grid_sie_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, workspace, mixed=None, stream=None):
+    return lt_gradient_grid_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, workspace, mixed, stream,
+                                 _fn="lt_gradient_grid_sie_host", _cols=5)
+
+
+def lt_gradient_points(lenses, points, out=None, workspace=None, stream=None, _fn="lt_gradient_points", _cols=7):
     """fp64 deflection at arbitrary points ([n, 2] float64 CUDA).  Returns [n, 2]."""
-    lenses = _lenses_dev(lenses)
+    lenses = _lenses_dev(lenses, _cols)
     n_lens = lenses.shape[0]
     if not (points.is_cuda and points.dtype == torch.float64):
         raise TypeError("points must be a CUDA float64 tensor [n, 2]")
@@ -210,12 +229,16 @@ def lt_gradient_points(lenses, points, out=None, workspace=None, stream=None):
         out = torch.empty((n, 2), dtype=torch.float64, device=points.device)
     if workspace is None:
         workspace = alloc_workspace(n_lens, 1, 1, LT_FP64, points.device)
-    rc = lib().lt_gradient_points(ctypes.c_void_p(lenses.data_ptr() if n_lens else None), n_lens,
-                                  ctypes.c_void_p(points.data_ptr() if n else None), n,
-                                  ctypes.c_void_p(out.data_ptr() if n else None),
-                                  ctypes.c_void_p(workspace.data_ptr()), workspace.numel(), _stream(stream))
-    _check(rc, "lt_gradient_points")
+    rc = getattr(lib(), _fn)(ctypes.c_void_p(lenses.data_ptr() if n_lens else None), n_lens,
+                             ctypes.c_void_p(points.data_ptr() if n else None), n,
+                             ctypes.c_void_p(out.data_ptr() if n else None),
+                             ctypes.c_void_p(workspace.data_ptr()), workspace.numel(), _stream(stream))
+    _check(rc, _fn)
     return out
+
+
+def lt_gradient_points_sie(lenses, points, out=None, workspace=None, stream=None):
+    return lt_gradient_points(lenses, points, out, workspace, stream, _fn="lt_gradient_points_sie", _cols=5)
 
 
 def lt_last_status(workspace, stream=None):
