@@ -139,7 +139,9 @@ int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_poin
  * The same call with HOST buffers (the end-to-end path of bench.py's `e2e` figure): enqueues, on cuda_stream, the
  * host->device copy of the n_lens lens structs from h_lenses, lt_gradient_grid, and the device->host copy of the
  * whole map into h_out_grad (nx*ny*2 elements, type per mode).  Asynchronous with respect to the host only if both
- * host buffers are pinned; the caller synchronises cuda_stream before reading h_out_grad.  The device staging
+ * host buffers are pinned; the caller synchronises cuda_stream before reading h_out_grad.  If h_out_grad is pinned
+ * (cudaHostAlloc / cudaHostRegister, 16-byte aligned) and the mode is not LT_MIXED, the gradient kernel stores the map
+ * into it directly over PCIe while it computes, and no separate device-to-host copy is enqueued.  The device staging
  * buffers for the catalogue and the map are carved from d_workspace, which must hold
  * lt_host_workspace_bytes(n_lens, nx, ny, mode) bytes (>= lt_workspace_bytes; 0 on bad sizes).
  */
@@ -152,8 +154,9 @@ int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens,
 /*
  * Launch-configuration knobs (process-wide; 0 = the library's default).  ppt64 / ppt32: pixels per thread of the
  * fp64 (1, 2, 4) and fp32 (1, 2, 4) grid kernels; chunk64 / chunk32: lens records staged in shared memory at a time;
- * ctas_per_sm: cap on resident CTAs per SM of the persistent grids; single_launch: 1 = one launch of the chosen variant
- * over the whole grid instead of whole waves plus a finer-grained rest.  Results do not depend on
+ * ctas_per_sm: cap on resident CTAs per SM of the persistent grids; single_launch: bit 0 = one launch of the chosen
+ * variant over the whole grid instead of whole waves plus a finer-grained rest, bit 1 = the host
+ * entry points always stage the map in device memory and copy it, even into a pinned buffer.  Results do not depend on
  * any of them except that the fp32 tile centre moves with the pixels per thread of the launch
  * that owns the pixel.  Returns LT_ERR_BAD_SIZE on a negative value.
  */

@@ -22,7 +22,7 @@ namespace {
 thread_local int g_last_cuda_error = 0;
 
 struct Tuning {
-  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0;
+  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0, staged_host_output = 0;
 };
 Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
@@ -442,9 +442,22 @@ int gradient_grid_host_impl(const void* h_lenses, int n_lens, double x_min, doub
   void* d_out = ws + w + align_up(lens_bytes);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (n_lens > 0) LT_CUDA(cudaMemcpyAsync(d_lenses, h_lenses, lens_bytes, cudaMemcpyHostToDevice, st));
-  const int rc = gradient_grid_impl<M>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out, ws, w, st);
+  // A pinned (page-locked, hence device-mapped under UVA) output buffer is written by the gradient kernel itself: its
+  // warp-wide 512 B / 256 B stores go straight over PCIe while the kernel computes, instead of a device-to-host copy of
+  // the whole map after it.  Not for LT_MIXED (every pixel would cross twice) and not for pageable memory.
+  void* d_direct = nullptr;
+  if (mode != LT_MIXED && !g_tuning.staged_host_output) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, h_out_grad) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer &&
+        ((uintptr_t)at.devicePointer & 15) == 0)
+      d_direct = at.devicePointer;
+    else
+      (void)cudaGetLastError();
+  }
+  const int rc = gradient_grid_impl<M>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
+                                       d_direct ? d_direct : d_out, ws, w, st);
   if (rc != LT_OK) return rc;
-  LT_CUDA(cudaMemcpyAsync(h_out_grad, d_out, (size_t)nx * ny * elem, cudaMemcpyDeviceToHost, st));
+  if (!d_direct) LT_CUDA(cudaMemcpyAsync(h_out_grad, d_out, (size_t)nx * ny * elem, cudaMemcpyDeviceToHost, st));
   return LT_OK;
 }
 
@@ -486,7 +499,8 @@ int lt_last_launch_count(void) { return g_launches; }
 
 int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm, int single_launch) {
   if (ppt64 < 0 || ppt32 < 0 || chunk64 < 0 || chunk32 < 0 || ctas_per_sm < 0 || single_launch < 0) return LT_ERR_BAD_SIZE;
-  g_tuning.single_launch = single_launch;
+  g_tuning.single_launch = single_launch & 1;
+  g_tuning.staged_host_output = (single_launch >> 1) & 1;
   g_tuning.ppt64 = ppt64;
   g_tuning.ppt32 = ppt32;
   g_tuning.chunk64 = chunk64;

@@ -240,7 +240,21 @@ def test_host_buffer_entry_point(env):
         ws = lt.alloc_workspace(len(W.lenses), W.nx, W.ny, mode, host=True)
         lt.lt_gradient_grid_host(hL, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, hout, ws)
         torch.cuda.synchronize()
-        assert np.array_equal(hout.numpy(), _gpu_map(torch, lt, W, mode))
+        ref = _gpu_map(torch, lt, W, mode)
+        assert np.array_equal(hout.numpy(), ref)
+        # pageable output and the forced staging path give the same map as the kernel's direct stores into pinned memory
+        pageable = torch.full((W.ny, W.nx, 2), float("nan"), dtype=dt)
+        lt.lt_gradient_grid_host(hL, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, pageable, ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(pageable.numpy(), ref)
+        hout.fill_(float("nan"))
+        try:
+            lt.lt_set_tuning(single_launch=2)
+            lt.lt_gradient_grid_host(hL, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, hout, ws)
+            torch.cuda.synchronize()
+        finally:
+            lt.lt_set_tuning()
+        assert np.array_equal(hout.numpy(), ref)
 
 
 def test_row_block_sharding_stitches_to_the_unsharded_map(env):
