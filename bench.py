@@ -52,8 +52,8 @@ PAPER_V100_SIE = {"fp64": 6.9e10, "mixed": 8.2e10}
 # lanes per SM behind the "alu" peaks (paper's Table 1 convention: 2 ops/cycle x clock x lanes)
 LANES = {"fp64": 64, "fp32": 128, "mixed": 64}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at config 1, from the ncu --set full
-# capture summarised in profiles/ (r01_*); None until captured.
-NCU_TRAFFIC_BYTES = {"fp64": None, "fp32": None, "mixed": None}
+# capture summarised in profiles/r01d_ncu_full_summary.md (dPIE kernels at config 1; reads only: the map stays in L2).
+NCU_TRAFFIC_BYTES = {"fp64": 30464, "fp32": 35328, "mixed": 3483648}
 KERNEL_NAME = {"fp64": "lt_grad_f64_kernel", "fp32": "lt_grad_f32_kernel", "mixed": "lt_grad_list_f64_kernel"}
 
 
