@@ -334,13 +334,19 @@ def run_ours(args, W):
     ms_kernel_main = r.ms_kernel        # dominant kernel, events recorded by the library inside the timed steps
     sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0)
 
+    def traffic(mode):
+        # per launch of the dominant kernel, from the ncu --set full captures under profiles/ (None where not captured)
+        if args.model == "sie":
+            return 5876736 + 665637120 if mode == "fp64" else None
+        return NCU_TRAFFIC_BYTES[mode] if (args.config == 1 and not args.paper_regime) else None
+
     def roofline(mode, ms_k, units, flagged=1.0):
         # mixed: the dominant kernel is the fp64 recompute, which processes the flagged pixels only
         units = units * flagged
         peak = 2.0 * sms * LANES[mode] * sm_max * 1e6 / 1e12
         ach = r.f_nom * units / (ms_k * 1e-3) / 1e12
         return {"bound": "alu", "kernel": KERNEL_NAME[mode], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES[mode],
+                "frac": ach / peak, "traffic": traffic(mode),
                 "peak_source": "derived: 2 x %d SMs x %d lanes x %.0f MHz (DESIGN.md section 8); no FP%s vector peak in "
                                "MEASURED_PEAKS.json (%s)" % (sms, LANES[mode], sm_max, "64" if LANES[mode] == 64 else "32",
                                                              peak_src),
