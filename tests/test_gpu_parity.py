@@ -151,6 +151,37 @@ def test_full_size_cfg1_sampled_and_points(env):
     assert _err(g32, g64) < TOL_F32
 
 
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_full_size_configs_sampled(env, cfg):
+    """BASELINE configs 2, 3 and 4 (the precision stress case) at full size: 20000 random pixels plus the pixels nearest
+    every lens centre against the oracle in fp64 and fp32; the whole fp32 map against the oracle-checked fp64 map; the
+    whole mixed map = fp64 bits on flagged pixels, fp32 value elsewhere."""
+    torch, lt, O = env
+    W = workloads.make(cfg)
+    ws = []
+    g64 = _gpu_map(torch, lt, W, lt.LT_FP64)
+    g32 = _gpu_map(torch, lt, W, lt.LT_FP32)
+    rng = np.random.default_rng(100 + cfg)
+    i, j = rng.integers(0, W.nx, 20000), rng.integers(0, W.ny, 20000)
+    ic = np.clip(np.round((W.lenses[:, 0] - W.x_min) / W.dx), 0, W.nx - 1).astype(np.int64)
+    jc = np.clip(np.round((W.lenses[:, 1] - W.y_min) / W.dx), 0, W.ny - 1).astype(np.int64)
+    i = np.concatenate([i, ic, np.clip(ic - 1, 0, W.nx - 1), [0, W.nx - 1]])
+    j = np.concatenate([j, jc, np.clip(jc + 1, 0, W.ny - 1), [W.ny - 1, 0]])
+    ref = O.gradient_points(W.lenses, W.x_min + i * W.dx, W.y_min + j * W.dx)
+    s = np.abs(ref).max(axis=0)
+    e64 = (np.abs(g64[j, i] - ref).max(axis=0) / s).max()
+    e32 = (np.abs(g32[j, i].astype(np.float64) - ref).max(axis=0) / s).max()
+    smax = np.abs(g64).reshape(-1, 2).max(axis=0)
+    e32_map = (np.abs(g32.astype(np.float64) - g64).reshape(-1, 2).max(axis=0) / smax).max()
+    print("cfg", cfg, "sampled fp64", e64, "fp32", e32, "fp32 map vs fp64 map", e32_map)
+    assert e64 < TOL_F64 and e32 < TOL_F32 and e32_map < TOL_F32
+    m = _gpu_map(torch, lt, W, lt.LT_MIXED, ws_out=ws)
+    f = lt.lt_mixed_last_flags(ws[0], len(W.lenses), W.nx, W.ny).cpu().numpy() != 0
+    st = lt.lt_mixed_last_stats(ws[0])
+    assert st["n_flagged"] == int(f.sum())
+    assert np.array_equal(m[f], g64[f]) and np.array_equal(m[~f], g32[~f].astype(np.float64))
+
+
 def test_mixed_mode_follows_the_rule(env):
     """Mixed mode on config 0 and on the paper-regime variant of config 1 (reduced grid): the flag mask equals the
     oracle's rule applied to the GPU's own fp32 map (bit-exact: both take the fp32 decisions in fp32), flagged pixels
