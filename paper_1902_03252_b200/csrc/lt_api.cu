@@ -12,7 +12,7 @@
 
 static_assert(sizeof(lt_lens) == sizeof(LtRawLens), "lt_lens and LtRawLens must have the same layout");
 static_assert(sizeof(lt_sie_lens) == sizeof(LtRawSie), "lt_sie_lens and LtRawSie must have the same layout");
-static_assert(sizeof(LtSieLens<double>) == 80 && sizeof(LtSieLens<float>) == 48, "SIE record sizes");
+static_assert(sizeof(LtSieLens<double>) == 48 && sizeof(LtSieLens<float>) == 32, "SIE record sizes");
 template <class M> struct Rec64 { typedef typename M::template Rec<double>::type type; };
 template <class M> struct Rec32 { typedef typename M::template Rec<float>::type type; };
 static_assert(sizeof(LtLens<double>) == 128 && sizeof(LtLens<float>) == 64, "lens record sizes");

@@ -60,20 +60,9 @@ __device__ __forceinline__ void lt_copy16(void* dst, const void* src, int count)
   for (int w = threadIdx.x; w < count; w += blockDim.x) d[w] = s[w];
 }
 
-// One interaction of lens model M given the sky-frame offset d1 = theta_1 - xc and the two per-row products
-// d2sx = d2 * sx, d2cy = d2 * cy (d2 = theta_2 - yc; shared by the pixels of a row): a3 (rotate, scaled: Alg. 1 l.5-6
-// with the model's factors folded into cos/sin), then the model's body and back rotation (a4-a6).
-template <class M, class T, class R>
-__device__ __forceinline__ void lt_model_interaction(const T d1, const T d2sx, const T d2cy, const R& L,
-                                                     const LtTables<T>& tab, T& G1, T& G2) {
-  const T X = lt_fma(d1, L.cx, d2sx);
-  const T Y = lt_fma(-d1, L.sy, d2cy);
-  M::template interact<T>(X, Y, L, tab, G1, G2);
-}
-
 // ------------------------------------------------------------------------------------------------ fp64 grid kernel
 // a2 pixel coordinate (x_min + i*dx, product and sum rounded separately, exactly as the API states it), a3-a6 per
-// lens (lt_interaction), a7 one double2 store per pixel.
+// lens (the model's interact_sky), a7 one double2 store per pixel.
 template <class M, int PPT, int MINB>
 __global__ void __launch_bounds__(LT_THREADS, MINB)
 lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ lens,
@@ -116,9 +105,9 @@ lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ le
       for (int k = 0; k < cnt; ++k) {
         const Rec L = sl[k];
         const double d2 = t2 - L.y0;                                // Alg. 1 l.4
-        const double d2sx = d2 * L.sx, d2cy = d2 * L.cy;
+        const auto row = M::template row<double>(d2, L);            // what the pixels of the row share
 #pragma unroll
-        for (int p = 0; p < PPT; ++p) lt_model_interaction<M, double>(t1[p] - L.x0, d2sx, d2cy, L, tab, G1[p], G2[p]);  // l.3, l.5-14
+        for (int p = 0; p < PPT; ++p) M::template interact_sky<double>(t1[p] - L.x0, row, L, tab, G1[p], G2[p]);  // l.3, l.5-14
       }
     }
     if (j < ny) {
@@ -153,6 +142,7 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
   constexpr int TILE_W = 32 * PPT;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   // in-tile offsets from the tile centre, in pixels (exact in fp32)
+  const float fdx = (float)dx;
   const float jl = (float)wrp - 0.5f * (float)(LT_TILE_H - 1);
   float il[PPT];
 #pragma unroll
@@ -177,21 +167,34 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
         Rec F = lens32[base + k];
         const Rec64& D = lens64[base + k];
         const double d1 = cx - D.x0, d2 = cy - D.y0;
-        F.x0 = (float)fma(d1, D.cx, d2 * D.sx);
-        F.y0 = (float)fma(-d1, D.sy, d2 * D.cy);
+        if constexpr (M::kSkyFrame32) {             // sky-frame offset of the tile centre from the lens centre
+          F.x0 = (float)d1;
+          F.y0 = (float)d2;
+        } else {                                    // (scaled) lens-frame position of the tile centre
+          F.x0 = (float)fma(d1, D.cx, d2 * D.sx);
+          F.y0 = (float)fma(-d1, D.sy, d2 * D.cy);
+        }
         sl[k] = F;
       }
       __syncthreads();
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
         const Rec L = sl[k];
-        const float xr = fmaf(jl, L.sx, L.x0);
-        const float yr = fmaf(jl, L.cy, L.y0);
+        if constexpr (M::kSkyFrame32) {
+          const float d2 = fmaf(jl, fdx, L.y0);
+          const auto row = M::template row<float>(d2, L);
 #pragma unroll
-        for (int p = 0; p < PPT; ++p) {
-          const float x = fmaf(il[p], L.cx, xr);
-          const float y = fmaf(-il[p], L.sy, yr);
-          M::template interact<float>(x, y, L, tab, G1[p], G2[p]);   // Alg. 1 l.7-14
+          for (int p = 0; p < PPT; ++p)
+            M::template interact_sky<float>(fmaf(il[p], fdx, L.x0), row, L, tab, G1[p], G2[p]);   // Alg. 1 l.3-14
+        } else {
+          const float xr = fmaf(jl, L.sx, L.x0);
+          const float yr = fmaf(jl, L.cy, L.y0);
+#pragma unroll
+          for (int p = 0; p < PPT; ++p) {
+            const float x = fmaf(il[p], L.cx, xr);
+            const float y = fmaf(-il[p], L.sy, yr);
+            M::template interact_lens<float>(x, y, L, tab, G1[p], G2[p]);   // Alg. 1 l.7-14
+          }
         }
       }
     }
@@ -208,7 +211,7 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
 // ------------------------------------------------------------------------------------------------ fp64 list kernel
 // Pixels taken from (a) the compacted list of flagged pixel indices of the mixed rule (a9; count read from the
 // workspace header on the device, no host round trip) or (b) an array of arbitrary points.  Uses the same
-// lt_interaction in the same lens order as the fp64 grid kernel: identical bits for identical pixels.
+// interact_sky in the same lens order as the fp64 grid kernel: identical bits for identical pixels.
 // Groups of 4 * 256 entries, 4 per thread (entries 256 apart, so list reads stay coalesced); a rest of at most one
 // 256-entry group per CTA after the whole waves runs one entry per thread (the count is only known on the device, so
 // the split is made here, not on the host).
@@ -257,7 +260,7 @@ __device__ __forceinline__ void lt_list_group(const typename M::template Rec<dou
 #pragma unroll
       for (int p = 0; p < PPT; ++p) {
         const double d2 = t2[p] - L.y0;
-        lt_model_interaction<M, double>(t1[p] - L.x0, d2 * L.sx, d2 * L.cy, L, tab, G1[p], G2[p]);
+        M::template interact_sky<double>(t1[p] - L.x0, M::template row<double>(d2, L), L, tab, G1[p], G2[p]);
       }
     }
   }

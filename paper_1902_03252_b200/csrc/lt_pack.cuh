@@ -79,71 +79,83 @@ struct LtRawSie {  // = lt_sie_lens of include/lt_gradient.h
   double x, y, e, phi, b0;
 };
 
-// Domain of the SIE (eq. 17-18 P:153-160 need 1 -+ eps > 0; the paper assumes eps << 1): |eps| < 1, all finite.
+// Domain of the SIE (eq. 17-18 P:153-160 need 1 -+ eps > 0; the paper assumes eps << 1): |eps| < 1, b0 >= 0
+// (eq. 22 P:183 is a square), all finite.
 LT_HD bool lt_sie_valid(const LtRawSie& r) {
   const bool fin = isfinite(r.x) && isfinite(r.y) && isfinite(r.e) && isfinite(r.phi) && isfinite(r.b0);
-  return fin && r.e > -1.0 && r.e < 1.0;
+  return fin && r.e > -1.0 && r.e < 1.0 && r.b0 >= 0.0;
 }
 LT_HD void lt_pack_sie(const LtRawSie& r, LtSieLens<double>& L) {
   double s, c;
   sincos(r.phi, &s, &c);
-  const double a1 = sqrt(1.0 - r.e), a2 = sqrt(1.0 + r.e);
+  const double a1 = 1.0 - r.e, a2 = 1.0 + r.e, b2 = r.b0 * r.b0;
   L.x0 = r.x;
   L.y0 = r.y;
-  L.cx = a1 * c;
-  L.sx = a1 * s;
-  L.cy = a2 * c;
-  L.sy = a2 * s;
-  L.k1 = r.b0 * a1 * c;
-  L.k2 = r.b0 * a2 * s;
-  L.k3 = r.b0 * a2 * c;
-  L.k4 = r.b0 * a1 * s;
+  L.q11 = b2 * fma(a1 * c, c, a2 * s * s);
+  L.q12 = b2 * (-2.0 * r.e * c * s);
+  L.q22 = b2 * fma(a1 * s, s, a2 * c * c);
+  L.pad = 0.0;
 }
 LT_HD void lt_poison_sie(LtSieLens<double>& L) {
   const double n = NAN;
-  L.x0 = L.y0 = L.cx = L.sx = L.cy = L.sy = L.k1 = L.k2 = L.k3 = L.k4 = n;
+  L.x0 = L.y0 = L.q11 = L.q12 = L.q22 = L.pad = n;
 }
-LT_HD void lt_round_sie(const LtSieLens<double>& D, double dx, LtSieLens<float>& F) {
+LT_HD void lt_round_sie(const LtSieLens<double>& D, double, LtSieLens<float>& F) {
   F.x0 = 0.f;
   F.y0 = 0.f;
-  F.cx = (float)(dx * D.cx);
-  F.sx = (float)(dx * D.sx);
-  F.cy = (float)(dx * D.cy);
-  F.sy = (float)(dx * D.sy);
-  F.k1 = (float)D.k1;
-  F.k2 = (float)D.k2;
-  F.k3 = (float)D.k3;
-  F.k4 = (float)D.k4;
+  F.q11 = (float)D.q11;
+  F.q12 = (float)D.q12;
+  F.q22 = (float)D.q22;
+  F.pad = 0.f;
 }
 
 // ================================================================================================ lens models
-// What the kernels of lt_kernels.cuh are instantiated with: the record types, the per-lens precompute and the
-// per-interaction body (both models take the scaled lens-frame coordinates X = d1 cx + d2 sx, Y = d2 cy - d1 sy).
+// What the kernels of lt_kernels.cuh are instantiated with: the record types, the per-lens precompute, the products of
+// d2 = theta_2 - yc that the pixels of a row share (row) and the per-interaction body given d1 = theta_1 - xc
+// (interact_sky).  kSkyFrame32: how the fp32 kernel forms its coordinates (DESIGN.md section 5 / 11): false = lens-frame
+// position of the tile centre + in-tile steps along the rotated axes (interact_lens), true = sky-frame offset of the
+// tile centre from the lens centre + in-tile steps of dx (interact_sky).
 struct LtDpieModel {
   typedef LtRawLens Raw;
   template <class T> struct Rec { typedef LtLens<T> type; };
+  template <class T> struct Row { T d2sx, d2cy; };
   static constexpr bool kTables = true;
+  static constexpr bool kSkyFrame32 = false;
   static LT_HD bool valid(const Raw& r) { return lt_lens_valid(r); }
   static LT_HD void pack(const Raw& r, LtLens<double>& L) { lt_pack_lens(r, L); }
   static LT_HD void poison(LtLens<double>& L) { lt_poison_lens(L); }
   static LT_HD void round(const LtLens<double>& D, double dx, LtLens<float>& F) { lt_round_lens(D, dx, F); }
+  template <class T> static LT_HD Row<T> row(const T d2, const LtLens<T>& L) { return Row<T>{d2 * L.sx, d2 * L.cy}; }
   template <class T>
-  static LT_HD void interact(const T X, const T Y, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
+  static LT_HD void interact_lens(const T X, const T Y, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
     T ax, ay;
     lt_dpie_body<T>(X, Y, L, tab, ax, ay);
     lt_accumulate<T>(ax, ay, L, G1, G2);
+  }
+  template <class T>
+  static LT_HD void interact_sky(const T d1, const Row<T>& r, const LtLens<T>& L, const LtTables<T>& tab, T& G1,
+                                 T& G2) {
+    const T X = lt_fma(d1, L.cx, r.d2sx);            // Alg. 1 l.5, times q/f
+    const T Y = lt_fma(-d1, L.sy, r.d2cy);           // Alg. 1 l.6, times 1/f
+    interact_lens<T>(X, Y, L, tab, G1, G2);
   }
 };
 struct LtSieModel {
   typedef LtRawSie Raw;
   template <class T> struct Rec { typedef LtSieLens<T> type; };
+  template <class T> struct Row { typedef LtSieRow<T> type; };
   static constexpr bool kTables = false;
+  static constexpr bool kSkyFrame32 = true;
   static LT_HD bool valid(const Raw& r) { return lt_sie_valid(r); }
   static LT_HD void pack(const Raw& r, LtSieLens<double>& L) { lt_pack_sie(r, L); }
   static LT_HD void poison(LtSieLens<double>& L) { lt_poison_sie(L); }
   static LT_HD void round(const LtSieLens<double>& D, double dx, LtSieLens<float>& F) { lt_round_sie(D, dx, F); }
+  template <class T> static LT_HD LtSieRow<T> row(const T d2, const LtSieLens<T>& L) { return lt_sie_row<T>(d2, L); }
   template <class T>
-  static LT_HD void interact(const T X, const T Y, const LtSieLens<T>& L, const LtTables<T>&, T& G1, T& G2) {
-    lt_sie_interact<T>(X, Y, L, G1, G2);
+  static LT_HD void interact_lens(const T, const T, const LtSieLens<T>&, const LtTables<T>&, T&, T&) {}   // unused
+  template <class T>
+  static LT_HD void interact_sky(const T d1, const LtSieRow<T>& r, const LtSieLens<T>& L, const LtTables<T>&, T& G1,
+                                 T& G2) {
+    lt_sie_interact<T>(d1, r, L, G1, G2);
   }
 };
