@@ -66,6 +66,9 @@ def parse_args():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = the metric's)")
     ap.add_argument("--mode", default="fp64", choices=list(MODES))
     ap.add_argument("--paper-regime", action="store_true", help="light galaxy halos (DESIGN.md section 4)")
+    ap.add_argument("--m-max", type=float, default=0.0,
+                    help="mixed mode with a calibrated rule (paper_1902_03252_b200.calibrate): this M_max, "
+                         "c28 = (1 - 1/M_max)/2, minimal centre patches; 0 = the paper's constants")
     ap.add_argument("--model", default="dpie", choices=["dpie", "sie"],
                     help="dpie: BASELINE.json configs (headline); sie: the paper's Algorithm 1 on its benchmark "
                          "workload, 6730^2 pixels x 702 halos (SURVEY 8(f) NEXT-1)")
@@ -220,6 +223,8 @@ class Runner:
         self.grid_host = lt.lt_gradient_grid_sie_host if self.sie else lt.lt_gradient_grid_host
         # SIE: the paper's rule at its own pixel size; cluster-scale = b0 >= 1" (its cluster halos: 28.8", 14.1")
         self.mixed = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0) if self.sie else None
+        if M_MAX > 0:
+            self.mixed = (M_MAX, 0.5 * (1.0 - 1.0 / M_MAX), 0.0, 0.0, 1e300)
         self.d_lenses = torch.from_numpy(W.lenses).cuda()
         dt = torch.float32 if mode == "fp32" else torch.float64
         self.out = torch.empty((W.ny, W.nx, 2), dtype=dt, device="cuda")
@@ -360,7 +365,8 @@ def run_ours(args, W):
                                                                   args.mode in PAPER_V100_SIE) else None),
             "dtype": DTYPE[args.mode], "data": "synthetic",
             "config": {"workload": W.name, "n_lens": int(len(W.lenses)), "nx": W.nx, "ny": W.ny, "seed": W.seed,
-                       "mode": args.mode, "parallelism": "dp%d (independent catalogues, no exchange)" % world,
+                       "mode": args.mode, "mixed_rule": ("paper constants" if M_MAX <= 0 else "calibrated, M_max = %g" % M_MAX),
+                       "parallelism": "dp%d (independent catalogues, no exchange)" % world,
                        "l2": "256 MiB buffer overwritten between timed steps", "inputs": "resident in HBM"},
             "clocks": clocks,
             "e2e": {"value": world * r.units / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
@@ -408,8 +414,13 @@ def make_workload(args, seed_offset=0):
     return workloads.make(args.config, paper_regime=args.paper_regime, seed_offset=seed_offset)
 
 
+M_MAX = 0.0
+
+
 def main():
+    global M_MAX
     args = parse_args()
+    M_MAX = args.m_max
     if args.warmup < 3:
         args.warmup = 3
     from paper_1902_03252_b200 import workloads

@@ -1,0 +1,107 @@
+"""Empirical calibration of the paper's mixed-precision rule for a given catalogue.
+
+The paper derives its rule for the SIE analytically (Appendix A): an SP error bound E_SP = 2.3e-3" outside DP
+centre patches of 400 x 400 / 20 x 20 pixels, hence SP suffices where the magnification along an axis is
+M_i <= (dx/4)/E_SP = 3.26, and says that for other models the SP-safe fraction "has to be computed for each
+model independently".  This tool does that computation by measurement: it runs the fp32 and the fp64 kernels
+through the C ABI on the same catalogue and reports
+  * the SP error |fp32 - fp64| (arcsec) over the map, inside and outside the default centre patches, and as a function
+    of the distance to the nearest lens centre (in pixels) -- the dPIE analogue of Fig. 9;
+  * the magnification bound M_max = (dx/4)/E_SP it implies for this catalogue and pixel size (the paper's 3.26);
+  * the fraction of pixels that violate the paper's sufficiency criterion |err_i| <= dx/(4 M_i) in plain fp32, with M_i
+    from the fp64 map (M_i = dx/|dx - delta_i|, eq. 24-26), and how many of those the rule flags.
+
+    python -m paper_1902_03252_b200.calibrate --config 2 [--paper-regime] [--model sie]
+
+Marshalling and numpy post-processing only: every map comes from the CUDA kernels.  Needs a GPU.
+"""
+import argparse
+import json
+
+import numpy as np
+
+
+def _nearest_centre_px(W, lenses_xy, reach=128):
+    """Chebyshev distance (pixels) of every pixel to the nearest lens centre, exact up to `reach`, 1e9 beyond it"""
+    best = np.full((W.ny, W.nx), 1e9, dtype=np.float32)
+    for xc, yc in lenses_xy:
+        a, b = (xc - W.x_min) / W.dx, (yc - W.y_min) / W.dx
+        i0, i1 = max(int(np.floor(a)) - reach, 0), min(int(np.ceil(a)) + reach + 1, W.nx)
+        j0, j1 = max(int(np.floor(b)) - reach, 0), min(int(np.ceil(b)) + reach + 1, W.ny)
+        if i1 <= i0 or j1 <= j0:
+            continue
+        d = np.maximum(np.abs(np.arange(i0, i1)[None, :] - a), np.abs(np.arange(j0, j1)[:, None] - b)).astype(np.float32)
+        np.minimum(best[j0:j1, i0:i1], d, out=best[j0:j1, i0:i1])
+    return best
+
+
+def calibrate(W, model="dpie", mixed=None):
+    import torch
+    from . import lt
+    sie = model == "sie"
+    grid = lt.lt_gradient_grid_sie if sie else lt.lt_gradient_grid
+    L = torch.from_numpy(W.lenses).cuda()
+    g64 = grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_FP64).cpu().numpy()
+    g32 = grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_FP32).cpu().numpy().astype(np.float64)
+    ws = lt.alloc_workspace(len(W.lenses), W.nx, W.ny, lt.LT_MIXED)
+    grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_MIXED, mixed=mixed, workspace=ws)
+    flags = lt.lt_mixed_last_flags(ws, len(W.lenses), W.nx, W.ny).cpu().numpy()
+    err = np.abs(g32 - g64).max(axis=2)                       # arcsec, worse component
+    amax = float(np.abs(g64).max())
+    patch = (flags & 1) != 0
+    out = {"workload": W.name, "dx": W.dx, "max_abs_alpha": amax,
+           "sp_error_arcsec": {"max": float(err.max()), "p99.9": float(np.quantile(err, 0.999)),
+                               "median": float(np.median(err)),
+                               "max_inside_default_patches": float(err[patch].max()) if patch.any() else None,
+                               "max_outside_default_patches": float(err[~patch].max())},
+           "sp_error_rel_max": float(err.max() / amax)}
+    # error against the distance to the nearest centre
+    dist = _nearest_centre_px(W, W.lenses[:, :2])
+    edges = [0, 1, 2, 4, 8, 16, 32, 64, 128, 1e9]
+    out["max_sp_error_by_distance_px"] = {
+        "%g-%g" % (lo, hi): (float(err[(dist >= lo) & (dist < hi)].max()) if ((dist >= lo) & (dist < hi)).any() else None)
+        for lo, hi in zip(edges[:-1], edges[1:])}
+    e_sp = float(err.max())
+    out["implied_m_max_no_patches"] = W.dx / 4.0 / e_sp
+    out["implied_m_max_outside_default_patches"] = W.dx / 4.0 / float(err[~patch].max())
+    # the paper's sufficiency criterion with the axis magnifications of the fp64 map (backward differences, eq. 24)
+    d1 = np.empty_like(err); d2 = np.empty_like(err)
+    d1[:, 1:] = g64[:, 1:, 0] - g64[:, :-1, 0]; d1[:, 0] = d1[:, 1]
+    d2[1:, :] = g64[1:, :, 1] - g64[:-1, :, 1]; d2[0, :] = d2[1, :]
+    with np.errstate(divide="ignore"):
+        M = W.dx / np.minimum(np.abs(W.dx - d1), np.abs(W.dx - d2))     # the larger of the two axis magnifications
+    viol = err > W.dx / 4.0 / M
+    flagged = flags != 0
+    out["criterion"] = {"pixels_violating_in_plain_fp32": int(viol.sum()),
+                        "fraction_violating": float(viol.mean()),
+                        "violating_and_flagged_by_rule": int((viol & flagged).sum()),
+                        "violating_and_missed_by_rule": int((viol & ~flagged).sum()),
+                        "flagged_fraction": float(flagged.mean()), "patch_fraction": float(patch.mean())}
+    # the calibrated rule: M_max from the measured SP error with a safety factor of 2, eq. 28's constant re-derived the way
+    # the paper's own numbers are related (0.0104 = (0.03 - 0.0092)/2, i.e. c28 = (1 - 1/M_max)/2), minimal centre patches
+    m_cal = max(1.5, 0.5 * out["implied_m_max_no_patches"])
+    cal = (m_cal, 0.5 * (1.0 - 1.0 / m_cal), 0.0, 0.0, 1e300)
+    grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_MIXED, mixed=cal, workspace=ws)
+    f2 = lt.lt_mixed_last_flags(ws, len(W.lenses), W.nx, W.ny).cpu().numpy() != 0
+    out["calibrated_rule"] = {"m_max": m_cal, "c28": cal[1], "patch_halfwidths": [0.0, 0.0],
+                              "flagged_fraction": float(f2.mean()),
+                              "violating_and_missed": int((viol & ~f2).sum())}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--paper-regime", action="store_true")
+    ap.add_argument("--model", default="dpie", choices=["dpie", "sie"])
+    args = ap.parse_args()
+    from . import workloads
+    if args.model == "sie":
+        W, mixed = workloads.make_sie("paper"), (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0)
+    else:
+        W, mixed = workloads.make(args.config, paper_regime=args.paper_regime), None
+    print(json.dumps(calibrate(W, args.model, mixed)))
+
+
+if __name__ == "__main__":
+    main()
