@@ -314,3 +314,18 @@ def test_row_block_sharding_stitches_to_the_unsharded_map(env):
             assert np.abs(stitched - ref).max() / s < tol
             # blocks differ from the unsharded call by the rounding of their first row's coordinate only
             assert np.abs(stitched - whole).max() / s < (1e-13 if mode == lt.LT_FP64 else tol)
+
+
+def test_calibration_tool_on_small_workloads(env):
+    """paper_1902_03252_b200.calibrate: the rule, paper constants or calibrated, misses no pixel
+    that violates the paper's sufficiency criterion in plain fp32; the SP error is far below the fp32 tolerance."""
+    torch, lt, O = env
+    from paper_1902_03252_b200 import calibrate
+    for W, model, mixed in ((workloads.make(1, paper_regime=True, n_override=400), "dpie", None),
+                            (workloads.make_sie("small", n_override=300), "sie", (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0))):
+        r = calibrate.calibrate(W, model, mixed)
+        assert r["sp_error_rel_max"] < TOL_F32
+        assert r["criterion"]["violating_and_missed_by_rule"] == 0
+        assert r["calibrated_rule"]["violating_and_missed"] == 0
+        assert r["calibrated_rule"]["flagged_fraction"] <= r["criterion"]["flagged_fraction"] + 1e-12
+        assert r["implied_m_max_no_patches"] > 3.26
