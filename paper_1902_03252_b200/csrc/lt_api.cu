@@ -441,7 +441,20 @@ int gradient_grid_host_impl(const void* h_lenses, int n_lens, double x_min, doub
   void* d_lenses = ws + w;
   void* d_out = ws + w + align_up(lens_bytes);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (n_lens > 0) LT_CUDA(cudaMemcpyAsync(d_lenses, h_lenses, lens_bytes, cudaMemcpyHostToDevice, st));
+  // A pinned catalogue (a few KB) is read by the precompute kernel straight from host memory: one PCIe read instead of
+  // a copy-engine operation in front of the first kernel.  Pageable catalogues are copied.
+  const void* d_cat = d_lenses;
+  bool cat_direct = false;
+  if (n_lens > 0 && !g_tuning.staged_host_output) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, h_lenses) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer) {
+      d_cat = at.devicePointer;
+      cat_direct = true;
+    } else {
+      (void)cudaGetLastError();
+    }
+  }
+  if (n_lens > 0 && !cat_direct) LT_CUDA(cudaMemcpyAsync(d_lenses, h_lenses, lens_bytes, cudaMemcpyHostToDevice, st));
   // A pinned (page-locked, hence device-mapped under UVA) output buffer is written by the gradient kernel itself: its
   // warp-wide 512 B / 256 B stores go straight over PCIe while the kernel computes, instead of a device-to-host copy of
   // the whole map after it.  Not for LT_MIXED (every pixel would cross twice) and not for pageable memory.
@@ -454,7 +467,7 @@ int gradient_grid_host_impl(const void* h_lenses, int n_lens, double x_min, doub
     else
       (void)cudaGetLastError();
   }
-  const int rc = gradient_grid_impl<M>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
+  const int rc = gradient_grid_impl<M>(d_cat, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
                                        d_direct ? d_direct : d_out, ws, w, st);
   if (rc != LT_OK) return rc;
   if (!d_direct) LT_CUDA(cudaMemcpyAsync(h_out_grad, d_out, (size_t)nx * ny * elem, cudaMemcpyDeviceToHost, st));
