@@ -329,3 +329,37 @@ def test_calibration_tool_on_small_workloads(env):
         assert r["calibrated_rule"]["violating_and_missed"] == 0
         assert r["calibrated_rule"]["flagged_fraction"] <= r["criterion"]["flagged_fraction"] + 1e-12
         assert r["implied_m_max_no_patches"] > 3.26
+
+
+@pytest.mark.parametrize("name,emax,ratio,tol", [("e<=0.6, rcut/rcore 1.01-10", 0.6, (1.01, 10.0), 1e-12),
+                                                  ("e<=0.9", 0.9, (1.5, 1000.0), 1e-12),
+                                                  ("e<=0.99", 0.99, (1.5, 1000.0), 1e-12),
+                                                  ("rcut/rcore 1.0001-1.01", 0.6, (1.0001, 1.01), 1e-10)])
+def test_fp64_kernel_beyond_the_configs(env, name, emax, ratio, tol):
+    """Single lenses far outside the configs' parameter ranges (strong ellipticity, rcut close to rcore, rcore down to
+    1e-4", points from 1e-6" to 300" from the centre, a third of them on the lens axes) against the __float128 oracle
+    (no reflection).  Everything within 1e-12 except rcut/rcore -> 1, where the scale rcut/(rcut - rcore) amplifies the
+    rounding of psi_t - psi_c (outside every config; bound stated here)."""
+    torch, lt, O = env
+    rng = np.random.default_rng(5)
+    n = 8
+    L = np.empty((n, 7))
+    L[:, 0], L[:, 1] = rng.uniform(-100, 100, n), rng.uniform(-100, 100, n)
+    L[:, 2], L[:, 3] = rng.uniform(0, emax, n), rng.uniform(0, np.pi, n)
+    L[:, 4] = np.exp(rng.uniform(np.log(1e-4), np.log(10.0), n))
+    L[:, 5] = L[:, 4] * np.exp(rng.uniform(np.log(ratio[0]), np.log(ratio[1]), n))
+    L[:, 6] = rng.uniform(1, 10, n)
+    worst = 0.0
+    for k in range(n):
+        m = 4000
+        r = np.exp(rng.uniform(np.log(1e-6), np.log(300.0), m))
+        a = rng.uniform(0, 2 * np.pi, m)
+        a = np.where(rng.integers(0, 3, m) == 0, L[k, 3] + rng.integers(0, 4, m) * np.pi / 2, a)
+        px, py = L[k, 0] + r * np.cos(a), L[k, 1] + r * np.sin(a)
+        ref = O.gradient_points(L[k:k + 1], px, py, O.QUAD, reflect=False)
+        g = lt.lt_gradient_points(torch.from_numpy(L[k:k + 1]).cuda(),
+                                  torch.from_numpy(np.stack([px, py], 1)).cuda()).cpu().numpy()
+        assert np.isfinite(g).all()
+        worst = max(worst, np.abs(g - ref).max() / np.abs(ref).max())
+    print(name, "worst fp64 error / max|alpha|", worst)
+    assert worst < tol
