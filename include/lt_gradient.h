@@ -39,6 +39,7 @@ extern "C" {
 
 #define LT_VERSION 100
 #define LT_MAX_LENSES 65536
+#define LT_MAX_SOURCES 65536
 
 typedef struct {              /* one dPIE lens; fp64; lengths in arcsec, angle in radians                         */
   double x, y;                /* centre theta_center (Alg. 1 Require)                                      */
@@ -77,6 +78,14 @@ typedef struct {               /* mixed-rule constants; lt_mixed_defaults() give
   double patch_halfwidth_galaxy;    /* 0.3 arcsec =  20/2 px * 0.03"                                             */
   double b0_cluster_threshold;      /* lenses with b0 >= this are cluster-scale (15 arcsec, R15)                 */
 } lt_mixed_params;
+
+typedef struct {               /* one predicted image found by lt_find_images (32 bytes)                            */
+  int source;                  /* index into d_sources                                                              */
+  int cell;                    /* j*nx + i of the cell's lower-left node (i, j)                                     */
+  int triangle;                /* 0: nodes (i,j), (i+1,j), (i,j+1);  1: nodes (i+1,j+1), (i,j+1), (i+1,j)           */
+  int reserved;
+  double x, y;                 /* image-plane position with the barycentric coordinates of the source point        */
+} lt_image_hit;
 
 typedef struct {               /* filled by lt_mixed_last_stats */
   long long n_pixels;          /* -1: not recorded (the caller knows nx*ny)                                      */
@@ -150,6 +159,24 @@ int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens,
                           double x_min, double y_min, double dx, int nx, int ny,
                           lt_precision mode, const lt_mixed_params* mixed_or_null,
                           void* h_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * The consumer of the map in the paper's chi^2 algorithm (section 2.2.2, Fig. 1): every
+ * pixel -- the cell between four neighbouring nodes of the fp64 map d_grad ([ny, nx, 2], the output of lt_gradient_grid in
+ * LT_FP64 or LT_MIXED mode on the same grid) -- is cut into two triangles, each triangle is lensed into the source plane
+ * with beta = theta - dls_dos * gradPsi (eq. 13), and every (source point, triangle) pair whose source-plane
+ * triangle contains the point is appended to d_hits: a predicted multiple image, with its image-plane position by
+ * barycentric interpolation.  Triangles are closed (a point on a shared edge is reported by both neighbours); zero-area
+ * triangles contain nothing.  The inside test is exact fp64 arithmetic in a fixed order: the set of hits is reproducible
+ * bit for bit, their order in d_hits is not.
+ *   d_sources  device, n_sources * 2 doubles (beta_1, beta_2), 16-byte aligned; 0 <= n_sources <= LT_MAX_SOURCES
+ *   d_hits     device, max_hits records; d_n_hits: device int, set to the number of hits FOUND (zeroed first); if it
+ *              exceeds max_hits the surplus was counted but not stored.
+ * Asynchronous on cuda_stream; needs nx, ny >= 2.
+ */
+int lt_find_images(const double* d_grad, double x_min, double y_min, double dx, int nx, int ny, double dls_dos,
+                   const double* d_sources, int n_sources, lt_image_hit* d_hits, int max_hits, int* d_n_hits,
+                   void* cuda_stream);
 
 /*
  * Launch-configuration knobs (process-wide; 0 = the library's default).  ppt64 / ppt32: pixels per thread of the

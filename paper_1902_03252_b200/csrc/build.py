@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 PKG = os.path.dirname(HERE)
 LIB = os.path.join(PKG, "liblt_gradient.so")
 SOURCES = ["lt_api.cu"]
-DEPS = ["lt_api.cu", "lt_kernels.cuh", "lt_mixed.cuh", "lt_math.cuh", "lt_pack.cuh",
+DEPS = ["lt_api.cu", "lt_kernels.cuh", "lt_mixed.cuh", "lt_math.cuh", "lt_pack.cuh", "lt_images.cuh",
         os.path.join("..", "..", "include", "lt_gradient.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--fmad=false",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -9,8 +9,10 @@
 
 #include "../../include/lt_gradient.h"
 #include "lt_mixed.cuh"
+#include "lt_images.cuh"
 
 static_assert(sizeof(lt_lens) == sizeof(LtRawLens), "lt_lens and LtRawLens must have the same layout");
+static_assert(sizeof(lt_image_hit) == sizeof(LtImageHit) && sizeof(LtImageHit) == 32, "lt_image_hit layout");
 static_assert(sizeof(lt_sie_lens) == sizeof(LtRawSie), "lt_sie_lens and LtRawSie must have the same layout");
 static_assert(sizeof(LtSieLens<double>) == 48 && sizeof(LtSieLens<float>) == 32, "SIE record sizes");
 template <class M> struct Rec64 { typedef typename M::template Rec<double>::type type; };
@@ -577,6 +579,36 @@ int lt_gradient_grid_sie_host(const lt_sie_lens* h_lenses, int n_lens, double x_
                               void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
   return gradient_grid_host_impl<LtSieModel>(h_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
                                              h_out_grad, d_workspace, workspace_bytes, cuda_stream);
+}
+
+int lt_find_images(const double* d_grad, double x_min, double y_min, double dx, int nx, int ny, double dls_dos,
+                   const double* d_sources, int n_sources, lt_image_hit* d_hits, int max_hits, int* d_n_hits,
+                   void* cuda_stream) {
+  if (nx < 2 || ny < 2 || (long long)nx * ny >= (1LL << 31) || n_sources < 0 || n_sources > LT_MAX_SOURCES ||
+      max_hits < 0)
+    return LT_ERR_BAD_SIZE;
+  if (!d_grad || !d_n_hits || (n_sources > 0 && !d_sources) || (max_hits > 0 && !d_hits)) return LT_ERR_NULL_POINTER;
+  if (!(isfinite(x_min) && isfinite(y_min) && isfinite(dx) && isfinite(dls_dos)) || !(dx > 0.0)) return LT_ERR_BAD_GRID;
+  if (((uintptr_t)d_grad & 15) || ((uintptr_t)d_sources & 15) || ((uintptr_t)d_hits & 7)) return LT_ERR_MISALIGNED;
+  DeviceInfo dev;
+  const int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LT_CUDA(cudaMemsetAsync(d_n_hits, 0, sizeof(int), st));
+  if (n_sources == 0) return LT_OK;
+  const int tiles_x = (nx - 1 + 31) / 32, tiles_y = (ny - 1 + 7) / 8;
+  const long long n_tiles = (long long)tiles_x * tiles_y;
+  long long grid = (long long)dev.sms * 8;
+  if (grid > n_tiles) grid = n_tiles;
+  KernelEvents ke(st);
+  lt_find_images_kernel<<<(int)grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_grad), x_min, y_min, dx, nx, ny,
+                                                   dls_dos, reinterpret_cast<const double2*>(d_sources), n_sources,
+                                                   tiles_x, (int)n_tiles, reinterpret_cast<LtImageHit*>(d_hits), max_hits,
+                                                   d_n_hits);
+  LT_CUDA(cudaGetLastError());
+  ++g_launches;
+  return LT_OK;
 }
 
 int lt_last_status(const void* d_workspace, void* cuda_stream, int* bad_lens_or_null) {

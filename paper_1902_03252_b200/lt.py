@@ -21,7 +21,7 @@ _LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
 
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
-           "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host",
+           "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images",
            "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
 
 
@@ -77,6 +77,8 @@ def lib():
             getattr(L, name).restype = ci
         L.lt_gradient_points_sie.argtypes = L.lt_gradient_points.argtypes
         L.lt_gradient_points_sie.restype = ci
+        L.lt_find_images.argtypes = [vp, cd, cd, cd, ci, ci, cd, vp, ci, vp, ci, vp, vp]
+        L.lt_find_images.restype = ci
         L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci, ci]
         L.lt_last_launch_count.restype = ci
         L.lt_set_tuning.restype = ci
@@ -239,6 +241,40 @@ def lt_gradient_points(lenses, points, out=None, workspace=None, stream=None, _f
 
 def lt_gradient_points_sie(lenses, points, out=None, workspace=None, stream=None):
     return lt_gradient_points(lenses, points, out, workspace, stream, _fn="lt_gradient_points_sie", _cols=5)
+
+
+HIT_DTYPE = [("source", "i4"), ("cell", "i4"), ("triangle", "i4"), ("reserved", "i4"), ("x", "f8"), ("y", "f8")]
+
+
+def lt_find_images(grad, x_min, y_min, dx, dls_dos, sources, max_hits=1 << 16, hits=None, n_hits=None, stream=None):
+    """Predicted images of the source points `sources` ([n, 2] float64 CUDA) on the fp64 map `grad` ([ny, nx, 2] float64
+    CUDA).  Returns (hits, n_hits): a uint8 CUDA tensor [max_hits, 32] of lt_image_hit records and a 1-element int32
+    CUDA tensor with the number found.  Asynchronous; decode with hits_to_numpy after synchronising."""
+    if not (grad.is_cuda and grad.dtype == torch.float64 and grad.is_contiguous() and grad.dim() == 3):
+        raise TypeError("grad must be a contiguous CUDA float64 tensor [ny, nx, 2]")
+    ny, nx = grad.shape[0], grad.shape[1]
+    if not (sources.is_cuda and sources.dtype == torch.float64):
+        raise TypeError("sources must be a CUDA float64 tensor [n, 2]")
+    sources = sources.reshape(-1, 2).contiguous()
+    n = sources.shape[0]
+    if hits is None:
+        hits = torch.empty((max(int(max_hits), 1), 32), dtype=torch.uint8, device=grad.device)
+    if n_hits is None:
+        n_hits = torch.empty(1, dtype=torch.int32, device=grad.device)
+    rc = lib().lt_find_images(ctypes.c_void_p(grad.data_ptr()), float(x_min), float(y_min), float(dx), int(nx), int(ny),
+                              float(dls_dos), ctypes.c_void_p(sources.data_ptr() if n else None), n,
+                              ctypes.c_void_p(hits.data_ptr()), int(max_hits), ctypes.c_void_p(n_hits.data_ptr()),
+                              _stream(stream))
+    _check(rc, "lt_find_images")
+    return hits, n_hits
+
+
+def hits_to_numpy(hits, n_hits):
+    """(synchronises) the stored records as a numpy structured array sorted by (source, cell, triangle), and the count"""
+    import numpy as np
+    n = int(n_hits.item())
+    a = hits.cpu().numpy().view(np.dtype(HIT_DTYPE)).reshape(-1)[: min(n, hits.shape[0])]
+    return np.sort(a, order=["source", "cell", "triangle"]), n
 
 
 def lt_last_status(workspace, stream=None):

@@ -1,0 +1,90 @@
+"""GPU-vs-oracle parity of lt_find_images (the triangle search of the paper's section 2.2.2) through
+the C ABI: the SET of (source, cell, triangle) hits is bit-exact (index work; the inside test is exact fp64 arithmetic
+in a fixed order on both sides), the interpolated image positions agree to rounding."""
+import numpy as np
+import pytest
+
+from paper_1902_03252_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    from paper_1902_03252_b200 import lt
+    from oracle import find_images as F
+    lt.lib()
+    return torch, lt, F
+
+
+def _compare(torch, lt, F, g, x_min, y_min, dx, s, src, max_hits=1 << 16):
+    """g: CUDA fp64 map [ny, nx, 2] from the gradient kernel; oracle runs on a host copy of the same map"""
+    hits, n = lt.lt_find_images(g, x_min, y_min, dx, s, torch.from_numpy(src).cuda(), max_hits=max_hits)
+    got, n_found = lt.hits_to_numpy(hits, n)
+    ref = F.find_images(g.cpu().numpy(), x_min, y_min, dx, s, src)
+    assert n_found == len(ref)
+    if n_found <= max_hits:
+        for f in ("source", "cell", "triangle"):
+            assert np.array_equal(got[f], ref[f]), f
+        assert np.array_equal(got["x"], ref["x"]) and np.array_equal(got["y"], ref["y"])
+    return got, ref
+
+
+def test_dpie_cluster_reduced_grid(env):
+    """config 1 catalogue in the paper regime on a 301 x 287 grid (ragged tiles): 300 sources near the centre"""
+    torch, lt, F = env
+    W = workloads.make(1, paper_regime=True, n_override=301)
+    W = W._replace(ny=287)
+    g = lt.lt_gradient_grid(torch.from_numpy(W.lenses).cuda(), W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_FP64)
+    rng = np.random.default_rng(8)
+    src = rng.uniform(-15, 15, (300, 2))            # more than one shared-memory chunk of sources
+    got, ref = _compare(torch, lt, F, g, W.x_min, W.y_min, W.dx, 1.0, src)
+    counts = np.bincount(ref["source"], minlength=300)
+    print("images per source: min", counts.min(), "max", counts.max(), "total", len(ref))
+    assert counts.max() >= 3                        # strong lensing: some sources are multiply imaged
+    # D_LS/D_OS = 0.6 and a tiny hit buffer (overflow is counted, not stored)
+    _compare(torch, lt, F, g, W.x_min, W.y_min, W.dx, 0.6, src[:50])
+    hits, n = lt.lt_find_images(g, W.x_min, W.y_min, W.dx, 1.0, torch.from_numpy(src).cuda(), max_hits=5)
+    part, n_found = lt.hits_to_numpy(hits, n)
+    assert n_found == len(ref) and len(part) == 5
+
+
+def test_no_lens_nodes_and_edges(env):
+    """gradPsi = 0 with sources exactly on nodes, edges and the cut diagonal: the closed-triangle rule (R24) gives the
+    same multiple reports on both sides"""
+    torch, lt, F = env
+    nx, ny, dx, x0, y0 = 70, 19, 0.5, -3.0, 2.0
+    g = torch.zeros((ny, nx, 2), dtype=torch.float64, device="cuda")
+    src = np.array([[x0 + 4 * dx, y0 + 2 * dx], [x0 + 2.5 * dx, y0 + 3.5 * dx], [x0 + 10.25 * dx, y0 + 7 * dx],
+                    [x0, y0], [x0 + (nx - 1) * dx, y0 + (ny - 1) * dx], [x0 - 1.0, y0], [x0 + 33.3 * dx, y0 + 5.1 * dx]])
+    got, ref = _compare(torch, lt, F, g, x0, y0, dx, 1.0, src)
+    assert np.bincount(ref["source"], minlength=7).tolist() == [6, 2, 2, 1, 1, 0, 1]
+
+
+def test_sie_benchmark_full_size(env):
+    """The paper-like SIE benchmark map (6730 x 6730) with 8 sources: hit set bit-exact against the oracle"""
+    torch, lt, F = env
+    W = workloads.make_sie("paper")
+    g = lt.lt_gradient_grid_sie(torch.from_numpy(W.lenses).cuda(), W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_FP64)
+    rng = np.random.default_rng(12)
+    src = rng.normal(0.0, 8.0, (8, 2)) + W.lenses[0, :2]
+    got, ref = _compare(torch, lt, F, g, W.x_min, W.y_min, W.dx, 1.0, src)
+    print("SIE benchmark: images found", len(ref), "per source", np.bincount(ref["source"], minlength=8).tolist())
+    assert len(ref) >= 8
+
+
+def test_argument_errors(env):
+    torch, lt, F = env
+    g = torch.zeros((4, 4, 2), dtype=torch.float64, device="cuda")
+    s = torch.zeros((1, 2), dtype=torch.float64, device="cuda")
+    with pytest.raises(lt.LtError) as e:
+        lt.lt_find_images(g[:1].contiguous(), 0.0, 0.0, 1.0, 1.0, s)
+    assert e.value.code == -2
+    with pytest.raises(lt.LtError) as e:
+        lt.lt_find_images(g, 0.0, 0.0, 0.0, 1.0, s)
+    assert e.value.code == -3
+    hits, n = lt.lt_find_images(g, 0.0, 0.0, 1.0, 1.0, torch.zeros((0, 2), dtype=torch.float64, device="cuda"))
+    assert int(n.item()) == 0
