@@ -9,9 +9,10 @@
 //
 // One thread per cell, a CTA = 32 x 8 cells, persistent grid over the tiles.  The four corner deflections are read once
 // per cell (neighbouring threads and rows hit L1/L2: 16 B of DRAM traffic per node), beta = theta - (D_LS/D_OS) gradPsi is
-// formed in registers, and the loop over the sources (staged in shared memory, every lane reads the same entry) first
-// tests a conservatively rounded fp32 bounding box of the cell's source-plane image -- four compares on the FP32 pipe --
-// and only on a hit evaluates the exact fp64 edge functions.  All fp64 products and differences are written with
+// formed in registers, and the loop over the sources (staged in shared memory once per CTA, every lane reads the same
+// entry, four sources per step) tests a conservatively rounded fp32 bounding box of the cell's source-plane image --
+// four compares on the FP32 pipe -- and only on a hit evaluates the exact fp64 edge functions.  (Staging the tile's
+// nodes in shared memory instead was measured slower: two barriers per 256-cell tile cost more than the re-reads.)  All fp64 products and differences are written with
 // explicit round-to-nearest intrinsics in the order of the definition, so that the inside / outside decision is the
 // same bit for bit wherever it is evaluated.
 #pragma once
@@ -24,10 +25,9 @@ struct LtImageHit {          // = lt_image_hit of include/lt_gradient.h (32 byte
 
 #define LT_SRC_CHUNK 256
 
-struct LtSrcEntry {          // one source point in shared memory
-  double x, y;               // exact
-  float x_rd, x_ru, y_rd, y_ru;   // rounded down / up to fp32 for the conservative bounding-box test
-};
+// one source point in shared memory: the exact coordinates and, separately (one broadcast LDS.128 per source in the
+// hot loop), the coordinates rounded down / up to fp32 for the conservative bounding-box test
+struct LtSrcBox { float x_rd, x_ru, y_rd, y_ru; };
 
 __device__ __forceinline__ double lt_cross(double ux, double uy, double vx, double vy) {
   return __dsub_rn(__dmul_rn(ux, vy), __dmul_rn(uy, vx));
@@ -57,11 +57,12 @@ __device__ __forceinline__ void lt_test_triangle(double Ax, double Ay, double Bx
   hits[slot] = h;
 }
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_min, double dx, int nx, int ny,
                       double dls_dos, const double2* __restrict__ sources, int n_sources, int tiles_x, int n_tiles,
                       LtImageHit* __restrict__ hits, int max_hits, int* __restrict__ n_hits) {
-  __shared__ LtSrcEntry src[LT_SRC_CHUNK];
+  __shared__ LtSrcBox box[LT_SRC_CHUNK];
+  __shared__ double2 src[LT_SRC_CHUNK];
   const int lx = threadIdx.x & 31, ly = threadIdx.x >> 5;
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
@@ -83,32 +84,50 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
       b10x = __dsub_rn(t1b, __dmul_rn(dls_dos, g10.x)); b10y = __dsub_rn(t2a, __dmul_rn(dls_dos, g10.y));
       b01x = __dsub_rn(t1a, __dmul_rn(dls_dos, g01.x)); b01y = __dsub_rn(t2b, __dmul_rn(dls_dos, g01.y));
       b11x = __dsub_rn(t1b, __dmul_rn(dls_dos, g11.x)); b11y = __dsub_rn(t2b, __dmul_rn(dls_dos, g11.y));
-      lo_x = fminf(fminf(__double2float_rd(b00x), __double2float_rd(b10x)), fminf(__double2float_rd(b01x), __double2float_rd(b11x)));
-      hi_x = fmaxf(fmaxf(__double2float_ru(b00x), __double2float_ru(b10x)), fmaxf(__double2float_ru(b01x), __double2float_ru(b11x)));
-      lo_y = fminf(fminf(__double2float_rd(b00y), __double2float_rd(b10y)), fminf(__double2float_rd(b01y), __double2float_rd(b11y)));
-      hi_y = fmaxf(fmaxf(__double2float_ru(b00y), __double2float_ru(b10y)), fmaxf(__double2float_ru(b01y), __double2float_ru(b11y)));
+      // conservatively rounded fp32 bounding box: the exact min / max in fp64, then one rounding down / up
+      lo_x = __double2float_rd(fmin(fmin(b00x, b10x), fmin(b01x, b11x)));
+      hi_x = __double2float_ru(fmax(fmax(b00x, b10x), fmax(b01x, b11x)));
+      lo_y = __double2float_rd(fmin(fmin(b00y, b10y), fmin(b01y, b11y)));
+      hi_y = __double2float_ru(fmax(fmax(b00y, b10y), fmax(b01y, b11y)));
     }
     for (int base = 0; base < n_sources; base += LT_SRC_CHUNK) {
       const int cnt = min(LT_SRC_CHUNK, n_sources - base);
-      __syncthreads();
-      for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
-        const double2 s = sources[base + k];
-        LtSrcEntry e;
-        e.x = s.x; e.y = s.y;
-        e.x_rd = __double2float_rd(s.x); e.x_ru = __double2float_ru(s.x);
-        e.y_rd = __double2float_rd(s.y); e.y_ru = __double2float_ru(s.y);
-        src[k] = e;
+      if (n_sources > LT_SRC_CHUNK || tile == (int)blockIdx.x) {      // a single chunk is staged once per CTA
+        __syncthreads();
+        for (int k = threadIdx.x; k < LT_SRC_CHUNK; k += blockDim.x) {
+          if (k < cnt) {
+            const double2 s = sources[base + k];
+            src[k] = s;
+            box[k] = LtSrcBox{__double2float_rd(s.x), __double2float_ru(s.x), __double2float_rd(s.y), __double2float_ru(s.y)};
+          } else {
+            box[k] = LtSrcBox{0.f, -INFINITY, 0.f, -INFINITY};   // x_ru = -inf: fails against every box
+          }
+        }
+        __syncthreads();
       }
-      __syncthreads();
-      for (int k = 0; k < cnt; ++k) {
-        // conservative: P in [lo, hi] in exact arithmetic implies this test passes
-        if (src[k].x_ru >= lo_x && src[k].x_rd <= hi_x && src[k].y_ru >= lo_y && src[k].y_rd <= hi_y) {
-          const double Px = src[k].x, Py = src[k].y;
-          const int cell = j * nx + i;
-          lt_test_triangle(b00x, b00y, b10x, b10y, b01x, b01y, t1a, t2a, t1b, t2a, t1a, t2b, Px, Py, base + k, cell, 0,
-                           hits, max_hits, n_hits);
-          lt_test_triangle(b11x, b11y, b01x, b01y, b10x, b10y, t1b, t2b, t1a, t2b, t1b, t2a, Px, Py, base + k, cell, 1,
-                           hits, max_hits, n_hits);
+      // four sources per step: four independent broadcast loads and compare chains, one vote and one (rarely taken)
+      // branch for the group; the padding entries of the last group are boxes no cell can hit
+      for (int k0 = 0; k0 < cnt; k0 += 4) {
+        bool near[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const LtSrcBox b = box[k0 + u];
+          // conservative: P in [lo, hi] in exact arithmetic implies this test passes; one predicate, no short circuit
+          near[u] = (b.x_ru >= lo_x) & (b.x_rd <= hi_x) & (b.y_ru >= lo_y) & (b.y_rd <= hi_y);
+        }
+        if (__any_sync(0xffffffffu, near[0] | near[1] | near[2] | near[3])) {
+#pragma unroll 1
+          for (int u = 0; u < 4; ++u) {
+            if (near[u]) {
+              const int k = k0 + u;
+              const double Px = src[k].x, Py = src[k].y;
+              const int cell = j * nx + i;
+              lt_test_triangle(b00x, b00y, b10x, b10y, b01x, b01y, t1a, t2a, t1b, t2a, t1a, t2b, Px, Py, base + k,
+                               cell, 0, hits, max_hits, n_hits);
+              lt_test_triangle(b11x, b11y, b01x, b01y, b10x, b10y, t1b, t2b, t1a, t2b, t1b, t2a, Px, Py, base + k,
+                               cell, 1, hits, max_hits, n_hits);
+            }
+          }
         }
       }
     }
