@@ -12,9 +12,9 @@
 // formed in registers, and the loop over the sources (staged in shared memory once per CTA, every lane reads the same
 // entry, four sources per step) tests a conservatively rounded fp32 bounding box of the cell's source-plane image --
 // four compares on the FP32 pipe -- and only on a hit evaluates the exact fp64 edge functions.  (Staging the tile's
-// nodes in shared memory instead was measured slower: two barriers per 256-cell tile cost more than the re-reads.)  All fp64 products and differences are written with
-// explicit round-to-nearest intrinsics in the order of the definition, so that the inside / outside decision is the
-// same bit for bit wherever it is evaluated.
+// nodes in shared memory instead was measured slower: two barriers per 256-cell tile cost more than the re-reads.)
+// All fp64 products and differences are written with explicit round-to-nearest intrinsics in the order of the
+// definition, so that the inside / outside decision is the same bit for bit wherever it is evaluated.
 #pragma once
 #include <cuda_runtime.h>
 
