@@ -143,7 +143,6 @@ struct LtDpieModel {
 struct LtSieModel {
   typedef LtRawSie Raw;
   template <class T> struct Rec { typedef LtSieLens<T> type; };
-  template <class T> struct Row { typedef LtSieRow<T> type; };
   static constexpr bool kTables = false;
   static constexpr bool kSkyFrame32 = true;
   static LT_HD bool valid(const Raw& r) { return lt_sie_valid(r); }
