@@ -363,3 +363,35 @@ def test_fp64_kernel_beyond_the_configs(env, name, emax, ratio, tol):
         worst = max(worst, np.abs(g - ref).max() / np.abs(ref).max())
     print(name, "worst fp64 error / max|alpha|", worst)
     assert worst < tol
+
+
+def test_call_is_capturable_in_a_cuda_graph(env):
+    """The hot path enqueues only kernels and memsets on the caller's stream (no allocation, no synchronisation), so an
+    MCMC loop can capture it once in a CUDA graph and replay it with new catalogue contents in the same buffers."""
+    torch, lt, O = env
+    W = workloads.make(0)
+    L = torch.from_numpy(W.lenses).cuda()
+    for mode, dt in ((lt.LT_FP64, torch.float64), (lt.LT_MIXED, torch.float64)):
+        ws = lt.alloc_workspace(len(W.lenses), W.nx, W.ny, mode)
+        out = torch.empty((W.ny, W.nx, 2), dtype=dt, device="cuda")
+        lt.lt_gradient_grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, out=out, workspace=ws)   # warm-up (opt-ins)
+        torch.cuda.synchronize()
+        expect = out.clone()
+        g = torch.cuda.CUDAGraph()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            with torch.cuda.graph(g, stream=s):
+                lt.lt_gradient_grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, out=out, workspace=ws, stream=s)
+        out.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, expect)
+        # new parameters in the same device buffer: the replay follows them
+        L2 = W.lenses.copy()
+        L2[:, 6] *= 2.0
+        L.copy_(torch.from_numpy(L2).cuda())
+        g.replay()
+        torch.cuda.synchronize()
+        if mode == lt.LT_FP64:
+            assert torch.allclose(out, 2.0 * expect, rtol=1e-13, atol=0)
+        L.copy_(torch.from_numpy(W.lenses).cuda())
