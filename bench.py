@@ -387,6 +387,25 @@ def run_ours(args, W):
                         "roofline_frac_nominal": roofline(m, rm.ms_kernel, rm.units,
                                                           ex.get("flagged_fraction", 1.0))["frac"]}
         line["modes"] = modes
+        if rank == 0:
+            # the same step replayed from a CUDA graph (what an MCMC loop would do): launch gaps removed
+            gs = torch.cuda.Stream()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.stream(gs):
+                with torch.cuda.graph(graph, stream=gs):
+                    r.grid(r.d_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, r.code, mixed=r.mixed, out=r.out,
+                           workspace=r.ws, stream=gs)
+            ts = []
+            for it in range(13):
+                flush.fill_(1)
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                graph.replay()
+                b_.record()
+                torch.cuda.synchronize()
+                if it >= 3:
+                    ts.append(a.elapsed_time(b_))
+            line["cuda_graph_replay"] = {"ms_per_step": sum(ts) / len(ts), "value": r.units / (sum(ts) / len(ts) * 1e-3)}
         if rank == 0 and args.mode == "fp64":
             # the consumer of the map (section 2.2.2): triangle search for 64 synthetic source points on the
             # fp64 map just computed; memory-bound when the sources are few: 16 B per node read once
