@@ -149,8 +149,9 @@ int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_poin
  * host->device copy of the n_lens lens structs from h_lenses, lt_gradient_grid, and the device->host copy of the
  * whole map into h_out_grad (nx*ny*2 elements, type per mode).  Asynchronous with respect to the host only if both
  * host buffers are pinned; the caller synchronises cuda_stream before reading h_out_grad.  If h_out_grad is pinned
- * (cudaHostAlloc / cudaHostRegister, 16-byte aligned) and the mode is not LT_MIXED, the gradient kernel stores the map
- * into it directly over PCIe while it computes, and no separate device-to-host copy is enqueued.  The device staging
+ * (cudaHostAlloc / cudaHostRegister, 16-byte aligned) the kernels store the map into it directly over PCIe while they
+ * compute (LT_MIXED: every pixel by the fp32 pass, flagged pixels again by the fp64 pass), and no separate
+ * device-to-host copy is enqueued.  The device staging
  * buffers for the catalogue and the map are carved from d_workspace, which must hold
  * lt_host_workspace_bytes(n_lens, nx, ny, mode) bytes (>= lt_workspace_bytes; 0 on bad sizes).
  */

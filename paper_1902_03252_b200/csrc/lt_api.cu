@@ -235,9 +235,8 @@ int launch_f64(const typename Rec64<M>::type* l64, const LtTables<double>* t64, 
 
 template <class M, int PPT, int MINB>
 int launch_f32_ppt(const typename Rec64<M>::type* l64, const typename Rec32<M>::type* l32, const LtTables<float>* t32,
-                   const GridArgs& a,
-                   float2* out, const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end,
-                   long long* resident) {
+                   const GridArgs& a, float2* out, double2* out_wide, const DeviceInfo& d, cudaStream_t st,
+                   int tiles_x, long long begin, long long end, long long* resident) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
                                sizeof(typename Rec32<M>::type), d);
   const size_t smem = (size_t)chunk * sizeof(typename Rec32<M>::type);
@@ -246,7 +245,7 @@ int launch_f32_ppt(const typename Rec64<M>::type* l64, const typename Rec32<M>::
   const int rc = grid_for(lt_grad_f32_kernel<M, PPT, MINB>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
   lt_grad_f32_kernel<M, PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
-                                                         a.ny, tiles_x, (int)begin, (int)end, out);
+                                                         a.ny, tiles_x, (int)begin, (int)end, out, out_wide);
   LT_CUDA(cudaGetLastError());
   ++g_launches;
   return LT_OK;
@@ -254,16 +253,16 @@ int launch_f32_ppt(const typename Rec64<M>::type* l64, const typename Rec32<M>::
 template <class M>
 int launch_f32(const typename Rec64<M>::type* l64, const typename Rec32<M>::type* l32, const LtTables<float>* t32,
                const GridArgs& a,
-               float2* out, const DeviceInfo& d, cudaStream_t st, bool hook = true) {
+               float2* out, const DeviceInfo& d, cudaStream_t st, bool hook = true, double2* out_wide = nullptr) {
   // 4 pixels per thread at <= 80 registers (3 CTAs per SM): with a tighter register budget the compiler reloads the
   // constants inside the loop and the kernel, which is bound by issue slots, loses 10 %
   KernelEvents ke(st, hook);
   return launch_waves(pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
                         switch (ppt) {
-                          case 1: return launch_f32_ppt<M, 1, 6>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
-                          case 2: return launch_f32_ppt<M, 2, 4>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
-                          default: return launch_f32_ppt<M, 4, 3>(l64, l32, t32, a, out, d, st, tiles_x, b, e, resident);
+                          case 1: return launch_f32_ppt<M, 1, 6>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                          case 2: return launch_f32_ppt<M, 2, 4>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                          default: return launch_f32_ppt<M, 4, 3>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
                         }
                       });
 }
@@ -390,13 +389,13 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
     LT_CUDA(cudaGetLastError());
     ++g_launches;
   }
-  rc = launch_f32<M>(l64, l32, t32, a, sp, dev, st, /*hook=*/false);
+  rc = launch_f32<M>(l64, l32, t32, a, sp, dev, st, /*hook=*/false, (double2*)d_out_grad);
   if (rc != LT_OK) return rc;
   {
     long long blocks = (n_pix + 255) / 256;
     const long long cap = (long long)dev.sms * 16;
     if (blocks > cap) blocks = cap;
-    lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, (double2*)d_out_grad, list, hdr);   /* a8 */
+    lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, list, hdr);   /* a8 */
     LT_CUDA(cudaGetLastError());
     ++g_launches;
   }
@@ -459,9 +458,10 @@ int gradient_grid_host_impl(const void* h_lenses, int n_lens, double x_min, doub
   if (n_lens > 0 && !cat_direct) LT_CUDA(cudaMemcpyAsync(d_lenses, h_lenses, lens_bytes, cudaMemcpyHostToDevice, st));
   // A pinned (page-locked, hence device-mapped under UVA) output buffer is written by the gradient kernel itself: its
   // warp-wide 512 B / 256 B stores go straight over PCIe while the kernel computes, instead of a device-to-host copy of
-  // the whole map after it.  Not for LT_MIXED (every pixel would cross twice) and not for pageable memory.
+  // the whole map after it (in LT_MIXED the fp32 pass stores the widened value of every pixel and the fp64 pass
+  // overwrites the flagged ones, both while computing).  Not for pageable memory.
   void* d_direct = nullptr;
-  if (mode != LT_MIXED && !g_tuning.staged_host_output) {
+  if (!g_tuning.staged_host_output) {
     cudaPointerAttributes at;
     if (cudaPointerGetAttributes(&at, h_out_grad) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer &&
         ((uintptr_t)at.devicePointer & 15) == 0)

@@ -132,7 +132,8 @@ __global__ void __launch_bounds__(LT_THREADS, MINB)
 lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ lens64,
                    const typename M::template Rec<float>::type* __restrict__ lens32,
                    const LtTables<float>* __restrict__ tables, int n_lens, int chunk, double x_min, double y_min,
-                   double dx, int nx, int ny, int tiles_x, int tile_begin, int tile_end, float2* __restrict__ out) {
+                   double dx, int nx, int ny, int tiles_x, int tile_begin, int tile_end, float2* __restrict__ out,
+                   double2* __restrict__ out_wide) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
   typedef typename M::template Rec<float>::type Rec;
   typedef typename M::template Rec<double>::type Rec64;
@@ -202,7 +203,11 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
 #pragma unroll
       for (int p = 0; p < PPT; ++p) {
         const int i = i0 + 32 * p;
-        if (i < nx) out[(size_t)j * nx + i] = make_float2(G1[p], G2[p]);
+        if (i < nx) {
+          out[(size_t)j * nx + i] = make_float2(G1[p], G2[p]);
+          // mixed mode (R17): the widened value goes straight to the fp64 output; the fp64 pass overwrites flagged pixels
+          if (out_wide) out_wide[(size_t)j * nx + i] = make_double2((double)G1[p], (double)G2[p]);
+        }
       }
     }
   }

@@ -41,12 +41,13 @@ __global__ void lt_patch_kernel(const Raw* __restrict__ raw, int n_lens, double 
   }
 }
 
-// a8, part 2: criteria on the fp32 map, merge with the patch bit, widen the fp32 value into the fp64 output (R17),
+// a8, part 2: criteria on the fp32 map, merge with the patch bit (the fp32 kernel has already written the widened fp32
+// values into the fp64 output, R17),
 // append flagged pixels to the compact list (warp-aggregated atomic; the order of the list is irrelevant because
 // every pixel is recomputed independently), count.
 __global__ void __launch_bounds__(256)
 lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags,
-               double2* __restrict__ out, unsigned int* __restrict__ list, LtWsHeader* __restrict__ hdr) {
+               unsigned int* __restrict__ list, LtWsHeader* __restrict__ hdr) {
   const size_t n_pix = (size_t)nx * ny;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   const unsigned lane = threadIdx.x & 31;
@@ -93,7 +94,6 @@ lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, uns
       if (c0 < mp.t25 || c1 < mp.t25) f |= 2;                     // eq. 25
       if (c2 > mp.t28 || c3 > mp.t28) f |= 4;                     // eq. 28
       flags[p] = f;
-      out[p] = make_double2((double)a.x, (double)a.y);
       c_patch += f & 1;
       c25 += (f >> 1) & 1;
       c28 += (f >> 2) & 1;
