@@ -371,7 +371,8 @@ def run_ours(args, W):
             "clocks": clocks,
             "e2e": {"value": world * r.units / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": r.h2d, "d2h_bytes_per_step": r.d2h,
-                    "api": "lt_gradient_grid_host (pinned host catalogue in, pinned host map out)"},
+                    "api": "lt_gradient_grid_host: pinned host catalogue read over PCIe by the precompute kernel, map stored into "
+                           "pinned host memory over PCIe by the gradient kernels while they compute (no staging copy)"},
             "gpu_launches": r.launches * args.steps, "gpu_launches_per_step": r.launches,
             "roofline": roofline(args.mode, ms_kernel_main, r.units, extra.get("flagged_fraction", 1.0))}
     line.update(extra)
