@@ -1,0 +1,37 @@
+"""bench.py's reference arm runs on CPU (it times the oracle): check the JSON line it prints against the contract
+(keys, metric, unit, config) for both lens models, and that ranks other than 0 print nothing."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _run(extra, env=None):
+    e = dict(os.environ)
+    e.update(env or {})
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "3",
+                        "--cpu-seconds", "0.2"] + extra, capture_output=True, text=True, env=e, timeout=600)
+    assert r.returncode == 0, r.stderr
+    return r.stdout.strip()
+
+
+@pytest.mark.parametrize("extra,workload", [([], "cfg1_1024x1024_100"), (["--model", "sie"], "sie_paper_6730x6730_702")])
+def test_reference_arm_line(extra, workload):
+    out = _run(extra)
+    lines = [l for l in out.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "lens_pixel_gradient_evals_per_s" and d["unit"] == "lens*pixel/s"
+    assert d["higher_is_better"] is True and d["n_gpus"] == 1 and d["steps"] == 1 and d["warmup"] == 3
+    assert d["config"]["workload"] == workload and d["value"] > 0 and d["ms_per_step"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1 and d["cpu_baseline"]["sample"]
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
+    assert d["gpu_launches"] == 0 and d["data"] == "synthetic"
+
+
+def test_reference_arm_other_ranks_are_silent():
+    assert _run([], env={"RANK": "1", "WORLD_SIZE": "2"}) == ""
