@@ -345,6 +345,20 @@ def run_ours(args, W):
             return 6376448 + 664593408 if mode == "fp64" else None
         return NCU_TRAFFIC_BYTES[mode] if (args.config == 1 and not args.paper_regime) else None
 
+    def executed(mode, ms_k, units):
+        """The same launch against the instruction floor of the pipe that bounds it: instructions per interaction counted
+        in the SASS of the 4-pixel inner loop (profiles/r01e_ncu_full_summary.md).  fp64 / mixed: FP64-pipe instructions,
+        each holding an SMSP's 16-lane FP64 pipe for 2 cycles; fp32: all instructions, one issue slot each."""
+        per = {("dpie", "fp64"): 61.75, ("dpie", "mixed"): 61.75, ("dpie", "fp32"): 62.75,
+               ("sie", "fp64"): 12.75, ("sie", "mixed"): 12.75, ("sie", "fp32"): None}[(args.model, mode)]
+        if per is None:
+            return None
+        cycles = per * (2.0 if mode != "fp32" else 1.0)
+        floor = sms * 4 * sm_max * 1e6 * 32 / cycles                   # interactions per second at 100 % of the pipe
+        return {"instructions_per_interaction": per, "pipe": "fp64 (2 cycles per warp instruction)" if mode != "fp32"
+                else "issue slots (1 per warp instruction)", "floor_interactions_per_s": floor,
+                "frac_of_floor": units / (ms_k * 1e-3) / floor}
+
     def roofline(mode, ms_k, units, flagged=1.0):
         # mixed: the dominant kernel is the fp64 recompute, which processes the flagged pixels only
         units = units * flagged
@@ -356,7 +370,7 @@ def run_ours(args, W):
                                "MEASURED_PEAKS.json (%s)" % (sms, LANES[mode], sm_max, "64" if LANES[mode] == 64 else "32",
                                                              peak_src),
                 "flops_per_interaction_nominal": r.f_nom, "duration_ms": ms_k,
-                "interactions_per_launch": units,
+                "interactions_per_launch": units, "executed": executed(mode, ms_k, units),
                 "algorithmic_bytes_per_launch": r.out.numel() * r.out.element_size()}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
