@@ -149,3 +149,28 @@ def make_sie(kind="paper", n_override=None, seed_offset=0):
         sig = rng.uniform(10.0, 15.0)
         out[2 + k] = (xc, yc, rng.uniform(0.0, 0.15), rng.uniform(0.0, np.pi), b0_from_sigma_v(sig))
     return Workload(name, out, x_min, y_min, dx, n, n, seed)
+
+
+# ---------------------------------------------------------------------------------------------- NFW
+# A catalogue of pseudo-elliptical NFW lenses is a float64 array [n_lens, 6]: (xc, yc, epsilon, Phi, kappa_s, rs).
+def make_nfw(n_override=None, seed_offset=0):
+    """Synthetic cluster of NFW halos on a 512 x 512 grid over [-100, 100]": 2 cluster-scale halos (kappa_s U(0.15, 0.3),
+    rs U(40, 80)", epsilon U(0, 0.2), centres U(-20, 20)^2) + 62 galaxy-scale halos (kappa_s U(0.02, 0.08), rs U(1, 5)",
+    epsilon U(0, 0.2), centres N(0, 40^2) redrawn until inside), angles U(0, pi); seed 3000."""
+    name, n, L, seed = "nfw_512x512_64", 512, 100.0, 3000 + int(seed_offset)
+    rng = np.random.default_rng(seed)
+    if n_override is not None:
+        n = int(n_override)
+        name += "_n%d" % n
+    x_min, y_min, dx = grid(n, L)
+    out = np.empty((64, 6))
+    for k in range(2):
+        out[k] = (rng.uniform(-20, 20), rng.uniform(-20, 20), rng.uniform(0.0, 0.2), rng.uniform(0.0, np.pi),
+                  rng.uniform(0.15, 0.3), rng.uniform(40.0, 80.0))
+    for k in range(2, 64):
+        while True:
+            xc, yc = rng.normal(0.0, 40.0, 2)
+            if abs(xc) < L and abs(yc) < L:
+                break
+        out[k] = (xc, yc, rng.uniform(0.0, 0.2), rng.uniform(0.0, np.pi), rng.uniform(0.02, 0.08), rng.uniform(1.0, 5.0))
+    return Workload(name, out, x_min, y_min, dx, n, n, seed)
