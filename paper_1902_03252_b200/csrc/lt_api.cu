@@ -13,6 +13,7 @@
 
 static_assert(sizeof(lt_lens) == sizeof(LtRawLens), "lt_lens and LtRawLens must have the same layout");
 static_assert(sizeof(lt_image_hit) == sizeof(LtImageHit) && sizeof(LtImageHit) == 32, "lt_image_hit layout");
+static_assert(sizeof(lt_nfw_lens) == sizeof(LtRawNfw), "lt_nfw_lens and LtRawNfw must have the same layout");
 static_assert(sizeof(lt_sie_lens) == sizeof(LtRawSie), "lt_sie_lens and LtRawSie must have the same layout");
 static_assert(sizeof(LtSieLens<double>) == 48 && sizeof(LtSieLens<float>) == 32, "SIE record sizes");
 template <class M> struct Rec64 { typedef typename M::template Rec<double>::type type; };
@@ -384,7 +385,7 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   md.b0_cluster = mp.b0_cluster_threshold;
   LT_CUDA(cudaMemsetAsync(flags, 0, (size_t)n_pix, st));
   if (n_lens > 0) {
-    lt_patch_kernel<typename M::Raw><<<n_lens, 256, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, x_min, y_min, dx,
+    lt_patch_kernel<M><<<n_lens, 256, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, x_min, y_min, dx,
                                             nx, ny, md, flags);
     LT_CUDA(cudaGetLastError());
     ++g_launches;
@@ -555,6 +556,24 @@ int lt_gradient_grid_sie(const lt_sie_lens* d_lenses, int n_lens, double x_min, 
                          size_t workspace_bytes, void* cuda_stream) {
   return gradient_grid_impl<LtSieModel>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out_grad,
                                         d_workspace, workspace_bytes, cuda_stream);
+}
+
+int lt_gradient_grid_nfw(const lt_nfw_lens* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                         lt_precision mode, const lt_mixed_params* mixed_or_null, void* d_out_grad, void* d_workspace,
+                         size_t workspace_bytes, void* cuda_stream) {
+  return gradient_grid_impl<LtNfwModel>(d_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null, d_out_grad,
+                                        d_workspace, workspace_bytes, cuda_stream);
+}
+int lt_gradient_points_nfw(const lt_nfw_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
+                           double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  return gradient_points_impl<LtNfwModel>(d_lenses, n_lens, d_points, n_points, d_out, d_workspace, workspace_bytes,
+                                          cuda_stream);
+}
+int lt_gradient_grid_nfw_host(const lt_nfw_lens* h_lenses, int n_lens, double x_min, double y_min, double dx, int nx,
+                              int ny, lt_precision mode, const lt_mixed_params* mixed_or_null, void* h_out_grad,
+                              void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+  return gradient_grid_host_impl<LtNfwModel>(h_lenses, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
+                                             h_out_grad, d_workspace, workspace_bytes, cuda_stream);
 }
 
 int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_points, long long n_points,

@@ -18,12 +18,12 @@ struct LtMixedDev {          // host-prepared constants of the rule
 // a8, part 1: one CTA per lens marks its DP patch: the box of half-width hp = max(1, ceil(h/dx)) pixels centred on the
 // pixel nearest the lens centre, clipped to the grid (R14); h by lens class (b0 >= threshold: cluster-scale, R15).
 // Overlapping patches write the same value, so plain stores are race-free in effect.
-template <class Raw>
-__global__ void lt_patch_kernel(const Raw* __restrict__ raw, int n_lens, double x_min, double y_min, double dx,
+template <class M>
+__global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_lens, double x_min, double y_min, double dx,
                                 int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags) {
   const int k = blockIdx.x;
   if (k >= n_lens) return;
-  const double xc = raw[k].x, yc = raw[k].y, b0 = raw[k].b0;
+  const double xc = raw[k].x, yc = raw[k].y, b0 = M::patch_scale(raw[k]);   // the lens's deflection scale (R15)
   if (!(isfinite(xc) && isfinite(yc))) return;
   const double h = (b0 >= mp.b0_cluster) ? mp.h_cluster : mp.h_galaxy;
   long long hp = (long long)ceil(h / dx);

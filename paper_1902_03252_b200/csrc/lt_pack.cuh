@@ -109,6 +109,38 @@ LT_HD void lt_round_sie(const LtSieLens<double>& D, double, LtSieLens<float>& F)
   F.pad = 0.f;
 }
 
+// ================================================================================================ NFW
+struct LtRawNfw {  // = lt_nfw_lens of include/lt_gradient.h
+  double x, y, e, phi, ks, rs;
+};
+LT_HD bool lt_nfw_valid(const LtRawNfw& r) {
+  const bool fin = isfinite(r.x) && isfinite(r.y) && isfinite(r.e) && isfinite(r.phi) && isfinite(r.ks) && isfinite(r.rs);
+  return fin && r.e > -1.0 && r.e < 1.0 && r.ks >= 0.0 && r.rs > 0.0;
+}
+LT_HD void lt_pack_nfw(const LtRawNfw& r, LtNfwLens<double>& L) {
+  double s, c;
+  sincos(r.phi, &s, &c);
+  const double a1 = 1.0 - r.e, a2 = 1.0 + r.e, ir2 = 1.0 / (r.rs * r.rs);
+  L.x0 = r.x;
+  L.y0 = r.y;
+  L.q11 = ir2 * fma(a1 * c, c, a2 * s * s);
+  L.q12 = ir2 * (-2.0 * r.e * c * s);
+  L.q22 = ir2 * fma(a1 * s, s, a2 * c * c);
+  L.amp = 4.0 * r.ks * r.rs * r.rs;
+}
+LT_HD void lt_poison_nfw(LtNfwLens<double>& L) {
+  const double n = NAN;
+  L.x0 = L.y0 = L.q11 = L.q12 = L.q22 = L.amp = n;
+}
+LT_HD void lt_round_nfw(const LtNfwLens<double>& D, double, LtNfwLens<float>& F) {
+  F.x0 = 0.f;
+  F.y0 = 0.f;
+  F.q11 = (float)D.q11;
+  F.q12 = (float)D.q12;
+  F.q22 = (float)D.q22;
+  F.amp = (float)D.amp;
+}
+
 // ================================================================================================ lens models
 // What the kernels of lt_kernels.cuh are instantiated with: the record types, the per-lens precompute, the products of
 // d2 = theta_2 - yc that the pixels of a row share (row) and the per-interaction body given d1 = theta_1 - xc
@@ -125,6 +157,7 @@ struct LtDpieModel {
   static LT_HD void pack(const Raw& r, LtLens<double>& L) { lt_pack_lens(r, L); }
   static LT_HD void poison(LtLens<double>& L) { lt_poison_lens(L); }
   static LT_HD void round(const LtLens<double>& D, double dx, LtLens<float>& F) { lt_round_lens(D, dx, F); }
+  static LT_HD double patch_scale(const Raw& r) { return r.b0; }
   template <class T> static LT_HD Row<T> row(const T d2, const LtLens<T>& L) { return Row<T>{d2 * L.sx, d2 * L.cy}; }
   template <class T>
   static LT_HD void interact_lens(const T X, const T Y, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
@@ -149,6 +182,7 @@ struct LtSieModel {
   static LT_HD void pack(const Raw& r, LtSieLens<double>& L) { lt_pack_sie(r, L); }
   static LT_HD void poison(LtSieLens<double>& L) { lt_poison_sie(L); }
   static LT_HD void round(const LtSieLens<double>& D, double dx, LtSieLens<float>& F) { lt_round_sie(D, dx, F); }
+  static LT_HD double patch_scale(const Raw& r) { return r.b0; }
   template <class T> static LT_HD LtSieRow<T> row(const T d2, const LtSieLens<T>& L) { return lt_sie_row<T>(d2, L); }
   template <class T>
   static LT_HD void interact_lens(const T, const T, const LtSieLens<T>&, const LtTables<T>&, T&, T&) {}   // unused
@@ -156,5 +190,26 @@ struct LtSieModel {
   static LT_HD void interact_sky(const T d1, const LtSieRow<T>& r, const LtSieLens<T>& L, const LtTables<T>&, T& G1,
                                  T& G2) {
     lt_sie_interact<T>(d1, r, L, G1, G2);
+  }
+};
+struct LtNfwModel {
+  typedef LtRawNfw Raw;
+  template <class T> struct Rec { typedef LtNfwLens<T> type; };
+  static constexpr bool kTables = true;
+  static constexpr bool kSkyFrame32 = true;
+  static LT_HD bool valid(const Raw& r) { return lt_nfw_valid(r); }
+  static LT_HD void pack(const Raw& r, LtNfwLens<double>& L) { lt_pack_nfw(r, L); }
+  static LT_HD void poison(LtNfwLens<double>& L) { lt_poison_nfw(L); }
+  static LT_HD void round(const LtNfwLens<double>& D, double dx, LtNfwLens<float>& F) { lt_round_nfw(D, dx, F); }
+  static LT_HD double patch_scale(const Raw& r) { return 4.0 * r.ks * r.rs; }
+  template <class T> static LT_HD LtSieRow<T> row(const T d2, const LtNfwLens<T>& L) {
+    return LtSieRow<T>{d2, L.q12 * d2, L.q22 * d2};
+  }
+  template <class T>
+  static LT_HD void interact_lens(const T, const T, const LtNfwLens<T>&, const LtTables<T>&, T&, T&) {}   // unused
+  template <class T>
+  static LT_HD void interact_sky(const T d1, const LtSieRow<T>& r, const LtNfwLens<T>& L, const LtTables<T>& tab, T& G1,
+                                 T& G2) {
+    lt_nfw_interact<T>(d1, r, L, tab, G1, G2);
   }
 };

@@ -22,6 +22,7 @@ _LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
            "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images",
+           "lt_gradient_grid_nfw", "lt_gradient_points_nfw", "lt_gradient_grid_nfw_host",
            "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
 
 
@@ -72,11 +73,12 @@ def lib():
         L.lt_gradient_grid_host.restype = ci
         L.lt_gradient_points.argtypes = [vp, ci, vp, cll, vp, vp, sz, vp]
         L.lt_gradient_points.restype = ci
-        for name in ("lt_gradient_grid_sie", "lt_gradient_grid_sie_host"):
+        for name in ("lt_gradient_grid_sie", "lt_gradient_grid_sie_host", "lt_gradient_grid_nfw", "lt_gradient_grid_nfw_host"):
             getattr(L, name).argtypes = L.lt_gradient_grid.argtypes
             getattr(L, name).restype = ci
-        L.lt_gradient_points_sie.argtypes = L.lt_gradient_points.argtypes
-        L.lt_gradient_points_sie.restype = ci
+        for name in ("lt_gradient_points_sie", "lt_gradient_points_nfw"):
+            getattr(L, name).argtypes = L.lt_gradient_points.argtypes
+            getattr(L, name).restype = ci
         L.lt_find_images.argtypes = [vp, cd, cd, cd, ci, ci, cd, vp, ci, vp, ci, vp, vp]
         L.lt_find_images.restype = ci
         L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci, ci]
@@ -237,6 +239,22 @@ def lt_gradient_points(lenses, points, out=None, workspace=None, stream=None, _f
                              ctypes.c_void_p(workspace.data_ptr()), workspace.numel(), _stream(stream))
     _check(rc, _fn)
     return out
+
+
+def lt_gradient_grid_nfw(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None, out=None, workspace=None,
+                         stream=None):
+    """The same for pseudo-elliptical NFW lenses; lenses: CUDA float64 [n_lens, 6] = (xc, yc, eps, Phi, kappa_s, rs)."""
+    return lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode, mixed, out, workspace, stream,
+                            _fn="lt_gradient_grid_nfw", _cols=6)
+
+
+def lt_gradient_grid_nfw_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, workspace, mixed=None, stream=None):
+    return lt_gradient_grid_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, workspace, mixed, stream,
+                                 _fn="lt_gradient_grid_nfw_host", _cols=6)
+
+
+def lt_gradient_points_nfw(lenses, points, out=None, workspace=None, stream=None):
+    return lt_gradient_points(lenses, points, out, workspace, stream, _fn="lt_gradient_points_nfw", _cols=6)
 
 
 def lt_gradient_points_sie(lenses, points, out=None, workspace=None, stream=None):
