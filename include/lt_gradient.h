@@ -190,6 +190,18 @@ int lt_gradient_grid_host(const lt_lens* h_lenses, int n_lens,
                           void* h_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * The mixed rule alone (section 3.2-3.3, eq. 24-28, patches P:284) applied to a single
+ * precision map the CALLER supplies: d_sp_map = nx*ny*2 floats (layout as the LT_FP32 output), d_centres = n_centres * 3
+ * doubles (x, y, deflection scale: b0, resp. 4 kappa_s rs) for the centre patches, d_flags = nx*ny bytes out (bit0 patch,
+ * bit1 eq. 25, bit2 eq. 28).  lt_gradient_grid in LT_MIXED mode runs exactly these kernels on its own fp32 map; this
+ * entry point exists so that the rule can be checked against its definition on any map.  d_workspace needs
+ * lt_workspace_bytes(0, nx, ny, LT_MIXED) bytes; lt_mixed_last_stats works on it afterwards.  Asynchronous.
+ */
+int lt_mixed_rule(const float* d_sp_map, double x_min, double y_min, double dx, int nx, int ny,
+                  const double* d_centres, int n_centres, const lt_mixed_params* mixed_or_null,
+                  unsigned char* d_flags, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
  * The consumer of the map in the paper's chi^2 algorithm (section 2.2.2, Fig. 1): every
  * pixel -- the cell between four neighbouring nodes of the fp64 map d_grad ([ny, nx, 2], the output of lt_gradient_grid in
  * LT_FP64 or LT_MIXED mode on the same grid) -- is cut into two triangles, each triangle is lensed into the source plane

@@ -600,6 +600,55 @@ int lt_gradient_grid_sie_host(const lt_sie_lens* h_lenses, int n_lens, double x_
                                              h_out_grad, d_workspace, workspace_bytes, cuda_stream);
 }
 
+int lt_mixed_rule(const float* d_sp_map, double x_min, double y_min, double dx, int nx, int ny, const double* d_centres,
+                  int n_centres, const lt_mixed_params* mixed_or_null, unsigned char* d_flags, void* d_workspace,
+                  size_t workspace_bytes, void* cuda_stream) {
+  if (!sizes_ok(n_centres, nx, ny)) return LT_ERR_BAD_SIZE;
+  if (!d_sp_map || !d_flags || !d_workspace || (n_centres > 0 && !d_centres)) return LT_ERR_NULL_POINTER;
+  if (!(isfinite(x_min) && isfinite(y_min) && isfinite(dx)) || !(dx > 0.0)) return LT_ERR_BAD_GRID;
+  if (((uintptr_t)d_sp_map & 7) || ((uintptr_t)d_workspace & 15)) return LT_ERR_MISALIGNED;
+  const long long n_pix = (long long)nx * ny;
+  const Layout L = make_layout(0, n_pix, true);
+  if (workspace_bytes < L.total) return LT_ERR_WORKSPACE_TOO_SMALL;
+  lt_mixed_params mp;
+  lt_mixed_defaults(&mp);
+  if (mixed_or_null) {
+    mp = *mixed_or_null;
+    const int rc = check_mixed(mp);
+    if (rc != LT_OK) return rc;
+  }
+  DeviceInfo dev;
+  const int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char* ws = (unsigned char*)d_workspace;
+  LT_CUDA(cudaMemsetAsync(ws + L.header, 0, sizeof(LtWsHeader), st));
+  LT_CUDA(cudaMemsetAsync(d_flags, 0, (size_t)n_pix, st));
+  LtMixedDev md;
+  md.fdx = (float)dx;
+  md.t25 = (float)(dx / mp.m_max);
+  md.t28 = (float)(mp.c28 * dx);
+  md.h_cluster = mp.patch_halfwidth_cluster;
+  md.h_galaxy = mp.patch_halfwidth_galaxy;
+  md.b0_cluster = mp.b0_cluster_threshold;
+  if (n_centres > 0) {
+    lt_patch_kernel<LtCentreModel><<<n_centres, 256, 0, st>>>(reinterpret_cast<const LtCentre*>(d_centres), n_centres,
+                                                              x_min, y_min, dx, nx, ny, md, d_flags);
+    LT_CUDA(cudaGetLastError());
+    ++g_launches;
+  }
+  long long blocks = (n_pix + 255) / 256;
+  const long long cap = (long long)dev.sms * 16;
+  if (blocks > cap) blocks = cap;
+  lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(reinterpret_cast<const float2*>(d_sp_map), nx, ny, md, d_flags,
+                                              reinterpret_cast<unsigned int*>(ws + L.list),
+                                              reinterpret_cast<LtWsHeader*>(ws + L.header));
+  LT_CUDA(cudaGetLastError());
+  ++g_launches;
+  return LT_OK;
+}
+
 int lt_find_images(const double* d_grad, double x_min, double y_min, double dx, int nx, int ny, double dls_dos,
                    const double* d_sources, int n_sources, lt_image_hit* d_hits, int max_hits, int* d_n_hits,
                    void* cuda_stream) {

@@ -8,6 +8,12 @@
 #pragma once
 #include "lt_kernels.cuh"
 
+struct LtCentre { double x, y, scale; };            // lt_mixed_rule: a lens as the rule sees it (centre, deflection scale)
+struct LtCentreModel {
+  typedef LtCentre Raw;
+  static __host__ __device__ double patch_scale(const Raw& r) { return r.scale; }
+};
+
 struct LtMixedDev {          // host-prepared constants of the rule
   float fdx;                 // (float)dx
   float t25;                 // (float)(dx / m_max)

@@ -21,7 +21,7 @@ _LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
 
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
-           "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images",
+           "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images", "lt_mixed_rule",
            "lt_gradient_grid_nfw", "lt_gradient_points_nfw", "lt_gradient_grid_nfw_host",
            "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
 
@@ -79,6 +79,8 @@ def lib():
         for name in ("lt_gradient_points_sie", "lt_gradient_points_nfw"):
             getattr(L, name).argtypes = L.lt_gradient_points.argtypes
             getattr(L, name).restype = ci
+        L.lt_mixed_rule.argtypes = [vp, cd, cd, cd, ci, ci, vp, ci, ctypes.POINTER(lt_mixed_params), vp, vp, sz, vp]
+        L.lt_mixed_rule.restype = ci
         L.lt_find_images.argtypes = [vp, cd, cd, cd, ci, ci, cd, vp, ci, vp, ci, vp, vp]
         L.lt_find_images.restype = ci
         L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci, ci]
@@ -259,6 +261,25 @@ def lt_gradient_points_nfw(lenses, points, out=None, workspace=None, stream=None
 
 def lt_gradient_points_sie(lenses, points, out=None, workspace=None, stream=None):
     return lt_gradient_points(lenses, points, out, workspace, stream, _fn="lt_gradient_points_sie", _cols=5)
+
+
+def lt_mixed_rule(sp_map, x_min, y_min, dx, centres, mixed=None, workspace=None, stream=None):
+    """The mixed rule on a caller-supplied single precision map ([ny, nx, 2] float32 CUDA); centres: [n, 3] float64 CUDA
+    (x, y, deflection scale).  Returns (flags uint8 [ny, nx], workspace)."""
+    if not (sp_map.is_cuda and sp_map.dtype == torch.float32 and sp_map.is_contiguous() and sp_map.dim() == 3):
+        raise TypeError("sp_map must be a contiguous CUDA float32 tensor [ny, nx, 2]")
+    ny, nx = sp_map.shape[0], sp_map.shape[1]
+    centres = centres.reshape(-1, 3).contiguous()
+    n = centres.shape[0]
+    if workspace is None:
+        workspace = alloc_workspace(0, nx, ny, LT_MIXED, sp_map.device)
+    flags = torch.empty((ny, nx), dtype=torch.uint8, device=sp_map.device)
+    rc = lib().lt_mixed_rule(ctypes.c_void_p(sp_map.data_ptr()), float(x_min), float(y_min), float(dx), int(nx), int(ny),
+                             ctypes.c_void_p(centres.data_ptr() if n else None), n, _mixed_ptr(mixed),
+                             ctypes.c_void_p(flags.data_ptr()), ctypes.c_void_p(workspace.data_ptr()), workspace.numel(),
+                             _stream(stream))
+    _check(rc, "lt_mixed_rule")
+    return flags, workspace
 
 
 HIT_DTYPE = [("source", "i4"), ("cell", "i4"), ("triangle", "i4"), ("reserved", "i4"), ("x", "f8"), ("y", "f8")]
