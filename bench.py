@@ -47,6 +47,9 @@ F_NOM = 69.0
 # SIE (Algorithm 1) under the same convention: translate 2 + rotate 6 + R^2 5 + g 4 (with (1 -+ eps) b0
 # precomputed: 2 mul, 2 div by R counted as mul by 1/R) + rotate back 6 + accumulate 2 = 25 flops + 1 rsqrt.
 F_NOM_SIE = 26.0
+# NFW (eq. 16-20 + the circular formula, same convention): translate 2 + rotate 6 + R^2 5 + x 1 + ln(x/2) 1 + F 4 + bracket
+# and scale 3 + eq. 20 8 + rotate back 6 + accumulate 2 = 38 flops + 8 specials (2 sqrt, 3 div, ln, arccosh/arccos, 1/x).
+F_NOM_NFW = 46.0
 # the paper's own numbers for the SIE benchmark workload (Table 2 P:364-373 -> BASELINE.md, derived throughput on V100)
 PAPER_V100_SIE = {"fp64": 6.9e10, "mixed": 8.2e10}
 # lanes per SM behind the "alu" peaks (paper's Table 1 convention: 2 ops/cycle x clock x lanes)
@@ -69,9 +72,10 @@ def parse_args():
     ap.add_argument("--m-max", type=float, default=0.0,
                     help="mixed mode with a calibrated rule (paper_1902_03252_b200.calibrate): this M_max, "
                          "c28 = (1 - 1/M_max)/2, minimal centre patches; 0 = the paper's constants")
-    ap.add_argument("--model", default="dpie", choices=["dpie", "sie"],
+    ap.add_argument("--model", default="dpie", choices=["dpie", "sie", "nfw"],
                     help="dpie: BASELINE.json configs (headline); sie: the paper's Algorithm 1 on its benchmark "
-                         "workload, 6730^2 pixels x 702 halos (SURVEY 8(f) NEXT-1)")
+                         "workload, 6730^2 pixels x 702 halos (SURVEY 8(f) NEXT-1); nfw: 2048^2 pixels x 64 "
+                         "pseudo-elliptical NFW halos (NEXT-4)")
     ap.add_argument("--no-extras", action="store_true", help="skip the other modes, cpu_baseline and peak probes")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU work of the oracle sample")
     return ap.parse_args()
@@ -154,6 +158,8 @@ def oracle_sample(W, cpu_seconds, ns_per_interaction=100.0):
     """Row stride so that the `double` oracle does about `cpu_seconds` of CPU work on this workload."""
     if W.lenses.shape[1] == 5:
         ns_per_interaction = 15.0                 # SIE: one sqrt, two divisions
+    if W.lenses.shape[1] == 6:
+        ns_per_interaction = 60.0                 # NFW: log, acosh / acos, two sqrt
     total = W.nx * W.ny * len(W.lenses) * ns_per_interaction * 1e-9
     stride = max(1, int(round(total / cpu_seconds)))
     rows = (W.ny + stride - 1) // stride
@@ -161,7 +167,9 @@ def oracle_sample(W, cpu_seconds, ns_per_interaction=100.0):
 
 
 def oracle_module(W):
-    if W.lenses.shape[1] == 5:
+    if W.lenses.shape[1] == 6:
+        from oracle import lt_oracle_nfw as O
+    elif W.lenses.shape[1] == 5:
         from oracle import lt_oracle_sie as O
     else:
         from oracle import lt_oracle as O
@@ -219,8 +227,10 @@ class Runner:
         self.code = MODES[mode]
         n = len(W.lenses)
         self.sie = W.lenses.shape[1] == 5
-        self.grid = lt.lt_gradient_grid_sie if self.sie else lt.lt_gradient_grid
-        self.grid_host = lt.lt_gradient_grid_sie_host if self.sie else lt.lt_gradient_grid_host
+        self.nfw = W.lenses.shape[1] == 6
+        self.grid = {5: lt.lt_gradient_grid_sie, 6: lt.lt_gradient_grid_nfw}.get(W.lenses.shape[1], lt.lt_gradient_grid)
+        self.grid_host = {5: lt.lt_gradient_grid_sie_host, 6: lt.lt_gradient_grid_nfw_host}.get(W.lenses.shape[1],
+                                                                                                lt.lt_gradient_grid_host)
         # SIE: the paper's rule at its own pixel size; cluster-scale = b0 >= 1" (its cluster halos: 28.8", 14.1")
         self.mixed = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0) if self.sie else None
         if M_MAX > 0:
@@ -234,7 +244,7 @@ class Runner:
         self.ws_host = lt.alloc_workspace(n, W.nx, W.ny, self.code, host=True)
         self.units = W.nx * W.ny * n
         self.h2d = self.h_lenses.numel() * 8
-        self.f_nom = F_NOM_SIE if self.sie else F_NOM
+        self.f_nom = F_NOM_SIE if self.sie else (F_NOM_NFW if self.nfw else F_NOM)
         self.d2h = self.h_out.numel() * self.h_out.element_size()
 
     def step(self):
@@ -341,6 +351,8 @@ def run_ours(args, W):
 
     def traffic(mode):
         # per launch of the dominant kernel, from the ncu --set full captures under profiles/ (None where not captured)
+        if args.model == "nfw":
+            return None
         if args.model == "sie":
             return 6376448 + 664593408 if mode == "fp64" else None
         return NCU_TRAFFIC_BYTES[mode] if (args.config == 1 and not args.paper_regime) else None
@@ -350,7 +362,7 @@ def run_ours(args, W):
         in the SASS of the 4-pixel inner loop (profiles/r01e_ncu_full_summary.md).  fp64 / mixed: FP64-pipe instructions,
         each holding an SMSP's 16-lane FP64 pipe for 2 cycles; fp32: all instructions, one issue slot each."""
         per = {("dpie", "fp64"): 61.75, ("dpie", "mixed"): 61.75, ("dpie", "fp32"): 62.75,
-               ("sie", "fp64"): 12.75, ("sie", "mixed"): 12.75, ("sie", "fp32"): None}[(args.model, mode)]
+               ("sie", "fp64"): 12.75, ("sie", "mixed"): 12.75, ("sie", "fp32"): None}.get((args.model, mode))
         if per is None:
             return None
         cycles = per * (2.0 if mode != "fp32" else 1.0)
@@ -474,6 +486,8 @@ def make_workload(args, seed_offset=0):
     from paper_1902_03252_b200 import workloads
     if args.model == "sie":
         return workloads.make_sie("paper", seed_offset=seed_offset)
+    if args.model == "nfw":
+        return workloads.make_nfw(n_override=2048, seed_offset=seed_offset)
     return workloads.make(args.config, paper_regime=args.paper_regime, seed_offset=seed_offset)
 
 

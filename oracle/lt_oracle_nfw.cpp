@@ -3,7 +3,8 @@
  *
  * Plain, slow CPU oracle for the deflection map of pseudo-elliptical NFW lenses: the generalisation the paper names at
  * P:385 ("other commonly used parametric lens models like the Navarro-Frenk-White (NFW) profile"; references P:456,
- * P:475-476), SURVEY 8(f) NEXT-4.  Only tests/ and __graft_entry__.smoke() may call it; it shares no code with
+ * P:475-476), SURVEY 8(f) NEXT-4.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may call it; it shares no code with
  * paper_1902_03252_b200/csrc.
  *
  * What it follows (P:n = /root/reference/PAPER.md line n):
@@ -111,12 +112,12 @@ void points_impl(const lto_nfw_lens* L, int n, const double* px, const double* p
 
 template <class T>
 void grid_impl(const lto_nfw_lens* L, int n, double x_min, double y_min, double dx, int nx, int ny, double* out,
-               int n_threads) {
+               int n_threads, int row_stride) {
 #ifdef _OPENMP
   if (n_threads > 0) omp_set_num_threads(n_threads);
 #endif
 #pragma omp parallel for schedule(dynamic)
-  for (int j = 0; j < ny; ++j)
+  for (int j = 0; j < ny; j += row_stride)
     for (int i = 0; i < nx; ++i) {
       const double t1 = x_min + i * dx, t2 = y_min + j * dx;
       T G1, G2;
@@ -130,14 +131,15 @@ void grid_impl(const lto_nfw_lens* L, int n, double x_min, double y_min, double 
 
 extern "C" {
 
-/* precision: 0 = long double (reference), 1 = double, 3 = __float128 (audit).  Returns 0, or -1 on a bad argument. */
+/* precision: 0 = long double (reference), 1 = double, 3 = __float128 (audit).  row_stride > 1 computes rows 0, stride,
+ * 2*stride, ... only.  Returns 0, or -1 on a bad argument. */
 int lt_oracle_nfw_gradient_grid(const lto_nfw_lens* lenses, int n_lens, double x_min, double y_min, double dx, int nx,
-                                int ny, int precision, double* out, int n_threads) {
-  if ((n_lens > 0 && !lenses) || n_lens < 0 || nx < 1 || ny < 1 || !out) return -1;
+                                int ny, int precision, double* out, int n_threads, int row_stride) {
+  if ((n_lens > 0 && !lenses) || n_lens < 0 || nx < 1 || ny < 1 || !out || row_stride < 1) return -1;
   switch (precision) {
-    case 0: grid_impl<long double>(lenses, n_lens, x_min, y_min, dx, nx, ny, out, n_threads); return 0;
-    case 1: grid_impl<double>(lenses, n_lens, x_min, y_min, dx, nx, ny, out, n_threads); return 0;
-    case 3: grid_impl<__float128>(lenses, n_lens, x_min, y_min, dx, nx, ny, out, n_threads); return 0;
+    case 0: grid_impl<long double>(lenses, n_lens, x_min, y_min, dx, nx, ny, out, n_threads, row_stride); return 0;
+    case 1: grid_impl<double>(lenses, n_lens, x_min, y_min, dx, nx, ny, out, n_threads, row_stride); return 0;
+    case 3: grid_impl<__float128>(lenses, n_lens, x_min, y_min, dx, nx, ny, out, n_threads, row_stride); return 0;
   }
   return -1;
 }

@@ -32,7 +32,7 @@ def lib():
         build()
         L = ctypes.CDLL(_LIB)
         vp, ci, cd, cll = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_longlong
-        L.lt_oracle_nfw_gradient_grid.argtypes = [vp, ci, cd, cd, cd, ci, ci, ci, vp, ci]
+        L.lt_oracle_nfw_gradient_grid.argtypes = [vp, ci, cd, cd, cd, ci, ci, ci, vp, ci, ci]
         L.lt_oracle_nfw_gradient_points.argtypes = [vp, ci, vp, vp, cll, ci, vp, ci]
         L.lt_oracle_nfw_potential_points.argtypes = [vp, ci, vp, vp, cll, vp]
         L.lt_oracle_nfw_kappa.argtypes = [cd, cd, cd]
@@ -53,11 +53,11 @@ def _pts(px, py):
     return px, py
 
 
-def gradient_grid(lenses, x_min, y_min, dx, nx, ny, precision=LONG_DOUBLE, n_threads=0):
+def gradient_grid(lenses, x_min, y_min, dx, nx, ny, precision=LONG_DOUBLE, n_threads=0, row_stride=1):
     a, n = _lenses(lenses)
-    out = np.empty((ny, nx, 2), dtype=np.float64)
+    out = np.full((ny, nx, 2), np.nan, dtype=np.float64)
     rc = lib().lt_oracle_nfw_gradient_grid(a.ctypes.data, n, float(x_min), float(y_min), float(dx), int(nx), int(ny),
-                                           int(precision), out.ctypes.data, int(n_threads))
+                                           int(precision), out.ctypes.data, int(n_threads), int(row_stride))
     if rc != 0:
         raise ValueError("lt_oracle_nfw_gradient_grid: bad argument")
     return out

@@ -19,7 +19,8 @@ def _run(extra, env=None):
     return r.stdout.strip()
 
 
-@pytest.mark.parametrize("extra,workload", [([], "cfg1_1024x1024_100"), (["--model", "sie"], "sie_paper_6730x6730_702")])
+@pytest.mark.parametrize("extra,workload", [([], "cfg1_1024x1024_100"), (["--model", "sie"], "sie_paper_6730x6730_702"),
+                                            (["--model", "nfw"], "nfw_512x512_64_n2048")])
 def test_reference_arm_line(extra, workload):
     out = _run(extra)
     lines = [l for l in out.splitlines() if l.startswith("{")]
