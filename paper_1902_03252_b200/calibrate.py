@@ -11,7 +11,7 @@ through the C ABI on the same catalogue and reports
   * the fraction of pixels that violate the paper's sufficiency criterion |err_i| <= dx/(4 M_i) in plain fp32, with M_i
     from the fp64 map (M_i = dx/|dx - delta_i|, eq. 24-26), and how many of those the rule flags.
 
-    python -m paper_1902_03252_b200.calibrate --config 2 [--paper-regime] [--model sie]
+    python -m paper_1902_03252_b200.calibrate --config 2 [--paper-regime] [--model sie|nfw]
 
 Marshalling and numpy post-processing only: every map comes from the CUDA kernels.  Needs a GPU.
 """
@@ -38,8 +38,7 @@ def _nearest_centre_px(W, lenses_xy, reach=128):
 def calibrate(W, model="dpie", mixed=None):
     import torch
     from . import lt
-    sie = model == "sie"
-    grid = lt.lt_gradient_grid_sie if sie else lt.lt_gradient_grid
+    grid = {"sie": lt.lt_gradient_grid_sie, "nfw": lt.lt_gradient_grid_nfw}.get(model, lt.lt_gradient_grid)
     L = torch.from_numpy(W.lenses).cuda()
     g64 = grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_FP64).cpu().numpy()
     g32 = grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_FP32).cpu().numpy().astype(np.float64)
@@ -93,11 +92,13 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--paper-regime", action="store_true")
-    ap.add_argument("--model", default="dpie", choices=["dpie", "sie"])
+    ap.add_argument("--model", default="dpie", choices=["dpie", "sie", "nfw"])
     args = ap.parse_args()
     from . import workloads
     if args.model == "sie":
         W, mixed = workloads.make_sie("paper"), (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0)
+    elif args.model == "nfw":
+        W, mixed = workloads.make_nfw(n_override=2048), None
     else:
         W, mixed = workloads.make(args.config, paper_regime=args.paper_regime), None
     print(json.dumps(calibrate(W, args.model, mixed)))
