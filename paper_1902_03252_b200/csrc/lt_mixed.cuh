@@ -49,7 +49,7 @@ __global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_l
 
 // a8, part 2: criteria on the fp32 map, merge with the patch bit (the fp32 kernel has already written the widened fp32
 // values into the fp64 output, R17),
-// append flagged pixels to the compact list (warp-aggregated atomic; the order of the list is irrelevant because
+// append flagged pixels to the compact list (CTA-aggregated atomic; the order of the list is irrelevant because
 // every pixel is recomputed independently), count.
 __global__ void __launch_bounds__(256)
 lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags,
@@ -58,9 +58,11 @@ lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, uns
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   const unsigned lane = threadIdx.x & 31;
   unsigned long long c_patch = 0, c25 = 0, c28 = 0;
-  // whole warps iterate together (the trip count is rounded up to a multiple of 32 pixels) so that the ballots below
-  // always see a full mask
-  const size_t n_round = (n_pix + 31) / 32 * 32;
+  // whole CTAs iterate together (the trip count is rounded up to a multiple of 256 pixels) so that the ballots see a full
+  // mask and the barriers below are reached by every thread
+  __shared__ unsigned int warp_cnt[8], warp_base[8];
+  const unsigned wrp = threadIdx.x >> 5;
+  const size_t n_round = (n_pix + 255) / 256 * 256;
   for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_round; p += stride) {
     const bool live = p < n_pix;
     unsigned char f = 0;
@@ -104,13 +106,20 @@ lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, uns
       c25 += (f >> 1) & 1;
       c28 += (f >> 2) & 1;
     }
+    // append: one atomic per CTA and iteration (the eight warps' counts are scanned in shared memory)
     const unsigned m = __ballot_sync(0xffffffffu, f != 0);
-    if (m) {
-      unsigned int basepos = 0;
-      if (lane == 0) basepos = atomicAdd(&hdr->list_count, (unsigned int)__popc(m));
-      basepos = __shfl_sync(0xffffffffu, basepos, 0);
-      if (f != 0) list[basepos + __popc(m & ((1u << lane) - 1u))] = (unsigned int)p;
+    if (lane == 0) warp_cnt[wrp] = (unsigned int)__popc(m);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      unsigned int tot = 0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) { warp_base[w] = tot; tot += warp_cnt[w]; }
+      const unsigned int cta_base = tot ? atomicAdd(&hdr->list_count, tot) : 0u;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) warp_base[w] += cta_base;
     }
+    __syncthreads();
+    if (f != 0) list[warp_base[wrp] + __popc(m & ((1u << lane) - 1u))] = (unsigned int)p;
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
