@@ -36,3 +36,30 @@ def test_reference_arm_line(extra, workload):
 
 def test_reference_arm_other_ranks_are_silent():
     assert _run([], env={"RANK": "1", "WORLD_SIZE": "2"}) == ""
+
+
+@pytest.mark.gpu
+def test_our_arm_line_on_the_gpu():
+    """The line bench.py prints for our arm carries every key of the contract (value, e2e with its byte counts,
+    gpu_launches, clocks, roofline with bound / achieved / peak / frac / traffic, cpu_baseline)."""
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "3", "--warmup", "3", "--cpu-seconds", "0.5"],
+                       capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert k in d, k
+    assert d["metric"] == "lens_pixel_gradient_evals_per_s" and d["dtype"] == "f64" and d["scaling"] == "weak"
+    assert d["config"]["workload"] == "cfg1_1024x1024_100" and d["vs_baseline"] is None
+    assert d["value"] > 1e10 and d["gpu_launches"] >= 2 * d["steps"]
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 100 * 56 and e["d2h_bytes_per_step"] == 1024 * 1024 * 16
+    rf = d["roofline"]
+    assert rf["bound"] == "alu" and rf["unit"] == "TFLOP/s" and abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-12
+    assert rf["traffic"] is not None and 0 < rf["frac"] < 1
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    assert set(d["modes"]) == {"fp64", "fp32", "mixed"}
+    assert "sm_mhz" in d["clocks"] and "reasons" in d["clocks"]
