@@ -234,18 +234,18 @@ int launch_f64(const typename Rec64<M>::type* l64, const LtTables<double>* t64, 
                       });
 }
 
-template <class M, int PPT, int MINB>
+template <class M, int PPT, int MINB, bool WIDE>
 int launch_f32_ppt(const typename Rec64<M>::type* l64, const typename Rec32<M>::type* l32, const LtTables<float>* t32,
                    const GridArgs& a, float2* out, double2* out_wide, const DeviceInfo& d, cudaStream_t st,
                    int tiles_x, long long begin, long long end, long long* resident) {
   const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
                                sizeof(typename Rec32<M>::type), d);
   const size_t smem = (size_t)chunk * sizeof(typename Rec32<M>::type);
-  if (resident) return resident_ctas(lt_grad_f32_kernel<M, PPT, MINB>, smem, d, *resident);
+  if (resident) return resident_ctas(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, smem, d, *resident);
   int grid = 1;
-  const int rc = grid_for(lt_grad_f32_kernel<M, PPT, MINB>, smem, end - begin, d, grid);
+  const int rc = grid_for(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  lt_grad_f32_kernel<M, PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
+  lt_grad_f32_kernel<M, PPT, MINB, WIDE><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
                                                          a.ny, tiles_x, (int)begin, (int)end, out, out_wide);
   LT_CUDA(cudaGetLastError());
   ++g_launches;
@@ -260,10 +260,17 @@ int launch_f32(const typename Rec64<M>::type* l64, const typename Rec32<M>::type
   KernelEvents ke(st, hook);
   return launch_waves(pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
+                        if (out_wide) {      // mixed mode: the kernel variant that also stores the widened value
+                          switch (ppt) {
+                            case 1: return launch_f32_ppt<M, 1, 6, true>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                            case 2: return launch_f32_ppt<M, 2, 4, true>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                            default: return launch_f32_ppt<M, 4, 3, true>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                          }
+                        }
                         switch (ppt) {
-                          case 1: return launch_f32_ppt<M, 1, 6>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
-                          case 2: return launch_f32_ppt<M, 2, 4>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
-                          default: return launch_f32_ppt<M, 4, 3>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                          case 1: return launch_f32_ppt<M, 1, 6, false>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                          case 2: return launch_f32_ppt<M, 2, 4, false>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                          default: return launch_f32_ppt<M, 4, 3, false>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
                         }
                       });
 }

@@ -127,7 +127,7 @@ lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ le
 //   x' = X0 + il*(dx cos) + jl*(dx sin),  y' = Y0 + jl*(dx cos) - il*(dx sin)      (Alg. 1 l.3-6 merged)
 // so the fp32 rounding of the coordinate is relative to the tile size, not to |theta| (the |theta_c|/|dtheta| term of
 // (A.65)).  All per-interaction arithmetic is FP32.
-template <class M, int PPT, int MINB>
+template <class M, int PPT, int MINB, bool WIDE>
 __global__ void __launch_bounds__(LT_THREADS, MINB)
 lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ lens64,
                    const typename M::template Rec<float>::type* __restrict__ lens32,
@@ -206,7 +206,7 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
         if (i < nx) {
           out[(size_t)j * nx + i] = make_float2(G1[p], G2[p]);
           // mixed mode (R17): the widened value goes straight to the fp64 output; the fp64 pass overwrites flagged pixels
-          if (out_wide) out_wide[(size_t)j * nx + i] = make_double2((double)G1[p], (double)G2[p]);
+          if (WIDE) out_wide[(size_t)j * nx + i] = make_double2((double)G1[p], (double)G2[p]);
         }
       }
     }
