@@ -1,0 +1,79 @@
+"""Properties of the CUDA path that hold at any size, for the three lens models (tier 3): superposition
+over lenses (eq. 14-15), permutation of the catalogue, translation of grid and lenses together, a quarter
+turn of the whole configuration.  No oracle involved: the maps are compared with each other."""
+import numpy as np
+import pytest
+
+from paper_1902_03252_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    from paper_1902_03252_b200 import lt
+    lt.lib()
+    return torch, lt
+
+
+def _models(lt):
+    return {"dpie": (lt.lt_gradient_grid, workloads.make(1, paper_regime=True, n_override=160), 3),
+            "sie": (lt.lt_gradient_grid_sie, workloads.make_sie("small", n_override=160), 3),
+            "nfw": (lt.lt_gradient_grid_nfw, workloads.make_nfw(n_override=160), 3)}
+
+
+def _map(torch, fn, lenses, W, mode=0, x_min=None, y_min=None, nx=None, ny=None):
+    L = torch.from_numpy(np.ascontiguousarray(lenses)).cuda()
+    out = fn(L, W.x_min if x_min is None else x_min, W.y_min if y_min is None else y_min, W.dx,
+             W.nx if nx is None else nx, W.ny if ny is None else ny, mode)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("model", ["dpie", "sie", "nfw"])
+def test_superposition_and_permutation(env, model):
+    torch, lt = env
+    fn, W, angle_col = _models(lt)[model]
+    n = len(W.lenses)
+    whole = _map(torch, fn, W.lenses, W)
+    s = np.abs(whole).max()
+    parts = _map(torch, fn, W.lenses[: n // 3], W) + _map(torch, fn, W.lenses[n // 3:], W)
+    assert np.abs(whole - parts).max() / s < 1e-14
+    perm = np.random.default_rng(1).permutation(n)
+    assert np.abs(_map(torch, fn, W.lenses[perm], W) - whole).max() / s < 1e-14
+    # fp32: the same up to single precision rounding
+    w32 = _map(torch, fn, W.lenses, W, mode=1)
+    assert np.abs(_map(torch, fn, W.lenses[perm], W, mode=1) - w32).max() / s < 5e-6
+    # an empty catalogue gives exactly zero, a doubled catalogue exactly twice the map's worth of terms
+    assert np.all(_map(torch, fn, W.lenses[:0], W) == 0)
+    assert np.abs(_map(torch, fn, np.concatenate([W.lenses, W.lenses]), W) - 2 * whole).max() / s < 1e-14
+
+
+@pytest.mark.parametrize("model", ["dpie", "sie", "nfw"])
+def test_translation_and_quarter_turn(env, model):
+    torch, lt = env
+    fn, W, angle_col = _models(lt)[model]
+    whole = _map(torch, fn, W.lenses, W)
+    s = np.abs(whole).max()
+    # shift grid and lenses by the same vector: theta - theta_center changes only by the rounding of the shifted numbers
+    sh = np.array([37.25, -18.5])
+    Ls = W.lenses.copy()
+    Ls[:, 0] += sh[0]; Ls[:, 1] += sh[1]
+    shifted = _map(torch, fn, Ls, W, x_min=W.x_min + sh[0], y_min=W.y_min + sh[1])
+    assert np.abs(shifted - whole).max() / s < 1e-12
+    # quarter turn about the origin: (x, y) -> (-y, x), Phi -> Phi + pi/2; the deflection turns with it
+    Lr = W.lenses.copy()
+    Lr[:, 0], Lr[:, 1] = -W.lenses[:, 1], W.lenses[:, 0]
+    Lr[:, angle_col] = W.lenses[:, angle_col] + np.pi / 2
+    # rotated grid: new pixel (i', j') sits at (x', y') = (-y_j, x_i): i' runs over -y (descending j), j' over x
+    xs = W.x_min + np.arange(W.nx) * W.dx
+    ys = W.y_min + np.arange(W.ny) * W.dx
+    rot = _map(torch, fn, Lr, W, x_min=-ys[-1], y_min=xs[0], nx=W.ny, ny=W.nx)
+    # rot[j', i'] with x' = -ys[-1] + i' dx = -y_j  ->  j = ny-1-i';  y' = xs[0] + j' dx = x_i  ->  i = j'
+    back = np.empty_like(whole)
+    back[..., 0] = rot[:, ::-1, 1].T          # alpha_x(x, y) =  alpha'_y(x', y')
+    back[..., 1] = -rot[:, ::-1, 0].T         # alpha_y(x, y) = -alpha'_x(x', y')
+    assert np.abs(back - whole).max() / s < 1e-12
