@@ -22,7 +22,7 @@
  *                      convergence kappa(x) = 2 kappa_s (1 - F(x)) / (x^2 - 1) (kappa(1) = 2 kappa_s / 3), potential
  *                      psi(x) = 2 kappa_s rs^2 [ ln^2(x/2) - arccosh^2(1/x) ] (x < 1), [ ln^2(x/2) + arccos^2(1/x) ] (x > 1)
  *                      (reading R26).  R = 0 contributes 0 (alpha -> 0 like x ln x).
- * Written literally.  The bracket ln(x/2) + F(x) cancels to O(x^2 ln x) for x << 1: in long double the deflection keeps
+ * Written literally except for F near x = 1 (see nfw_F).  The bracket ln(x/2) + F(x) cancels to O(x^2 ln x) for x << 1: in long double the deflection keeps
  * ~1e-19 * 8 / x absolute accuracy relative to 4 kappa_s rs, i.e. better than 1e-13 of the lens's peak deflection for
  * x > 1e-5; the __float128 instantiation audits that.
  */
@@ -49,7 +49,8 @@ template <class T> struct M {
   static T sqrt_(T v) { return std::sqrt(v); }
   static T log_(T v) { return std::log(v); }
   static T acosh_(T v) { return std::acosh(v); }
-  static T acos_(T v) { return std::acos(v); }
+  static T atanh_(T v) { return std::atanh(v); }
+  static T atan_(T v) { return std::atan(v); }
   static T sin_(T v) { return std::sin(v); }
   static T cos_(T v) { return std::cos(v); }
 };
@@ -58,14 +59,20 @@ template <> struct M<__float128> {
   static T sqrt_(T v) { return sqrtq(v); }
   static T log_(T v) { return logq(v); }
   static T acosh_(T v) { return acoshq(v); }
-  static T acos_(T v) { return acosq(v); }
+  static T atanh_(T v) { return atanhq(v); }
+  static T atan_(T v) { return atanq(v); }
   static T sin_(T v) { return sinq(v); }
   static T cos_(T v) { return cosq(v); }
 };
 
+/* F(x).  For x >= 1/2, arccosh(1/x) and arccos(1/x) are evaluated through the identities arccosh(1/x) = atanh(sqrt(1 - x^2)) and
+ * arccos(1/x) = atan(sqrt(x^2 - 1)) (x > 0): the same numbers, but the literal route through 1/x loses eps/|1 - x| near
+ * the scale radius (1.5e-13 of the peak deflection at |1 - x| ~ 1e-7 even in long double), while F itself is smooth
+ * there (F = 1 - 2(x-1)/3 + ...).  DESIGN.md reading R27; pinned against the literal formula in 40-digit arithmetic. */
 template <class T> T nfw_F(T x) {
-  if (x < T(1)) return M<T>::acosh_(T(1) / x) / M<T>::sqrt_(T(1) - x * x);
-  if (x > T(1)) return M<T>::acos_(T(1) / x) / M<T>::sqrt_(x * x - T(1));
+  if (x < T(0.5)) return M<T>::acosh_(T(1) / x) / M<T>::sqrt_(T(1) - x * x);      /* literal: well conditioned here */
+  if (x < T(1)) { const T s = M<T>::sqrt_((T(1) - x) * (T(1) + x)); return M<T>::atanh_(s) / s; }
+  if (x > T(1)) { const T s = M<T>::sqrt_((x - T(1)) * (x + T(1))); return M<T>::atan_(s) / s; }
   return T(1);
 }
 /* |alpha(R)| of the circular NFW lens */

@@ -42,6 +42,31 @@ def test_values_at_the_scale_radius_and_limits():
     assert np.abs(r - q).max() / (4 * ks * rs) < 1e-13
 
 
+def test_literal_formula_in_40_digits_incl_the_neighbourhood_of_the_scale_radius():
+    """Reading R27: the oracle evaluates arccosh(1/x), arccos(1/x) as atanh / atan of sqrt(|1 - x^2|).  The literal textbook
+    formula, in 40-digit arithmetic (mpmath), is the reference here -- including |1 - x| down to 1e-9, where the literal
+    route loses eps/|1 - x| in long double."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    ks, rs = 0.27, 41.0
+
+    def alpha(x):
+        x = mp.mpf(x)
+        if x < 1:
+            F = mp.acosh(1 / x) / mp.sqrt(1 - x * x)
+        elif x > 1:
+            F = mp.acos(1 / x) / mp.sqrt(x * x - 1)
+        else:
+            F = mp.mpf(1)
+        return 4 * mp.mpf(ks) * rs * (mp.log(x / 2) + F) / x
+    L = np.array([[0.0, 0.0, 0.0, 0.0, ks, rs]])
+    for x in (1e-3, 0.2, 0.5, 1 - 1e-3, 1 - 1e-6, 1 - 1e-9, 1 + 1e-9, 1 + 1e-6, 1 + 1e-3, 3.0, 250.0):
+        R = rs * x
+        exact = alpha(mp.mpf(R) / rs)                    # the x the oracle sees: R / rs with R the fp64 number
+        got = N.gradient_points(L, [R], [0.0])[0][0]
+        assert abs(got - float(exact)) <= 4e-16 * 4 * ks * rs, x
+
+
 def test_gradient_of_the_potential_by_finite_differences():
     """alpha = grad psi (eq. 2) for the pseudo-elliptical potential psi_eps(theta) = psi(R) (eq. 19)"""
     W = workloads.make_nfw()
