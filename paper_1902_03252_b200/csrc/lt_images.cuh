@@ -9,9 +9,10 @@
 //
 // One thread per cell, a CTA = 32 x 8 cells, persistent grid over the tiles.  The four corner deflections are read once
 // per cell (neighbouring threads and rows hit L1/L2: 16 B of DRAM traffic per node), beta = theta - (D_LS/D_OS) gradPsi is
-// formed in registers, and the loop over the sources (staged in shared memory once per CTA, every lane reads the same
-// entry, four sources per step) tests a conservatively rounded fp32 bounding box of the cell's source-plane image --
-// four compares on the FP32 pipe -- and only on a hit evaluates the exact fp64 edge functions.  (Staging the tile's
+// formed in registers.  The sources are staged in shared memory once per CTA with their coordinates rounded down / up to
+// fp32.  Culling is hierarchical and conservative: 32 sources at a time are tested, one per lane, against the bounding
+// box of the warp's 32 cells; the survivors (usually none) against the cell's own conservatively rounded fp32 box --
+// four compares on the FP32 pipe -- and only on a hit the exact fp64 edge functions are evaluated.  (Staging the tile's
 // nodes in shared memory instead was measured slower: two barriers per 256-cell tile cost more than the re-reads.)
 // All fp64 products and differences are written with explicit round-to-nearest intrinsics in the order of the
 // definition, so that the inside / outside decision is the same bit for bit wherever it is evaluated.
@@ -63,7 +64,7 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
                       LtImageHit* __restrict__ hits, int max_hits, int* __restrict__ n_hits) {
   __shared__ LtSrcBox box[LT_SRC_CHUNK];
   __shared__ double2 src[LT_SRC_CHUNK];
-  const int lx = threadIdx.x & 31, ly = threadIdx.x >> 5;
+  const int lx = threadIdx.x & 31, ly = threadIdx.x >> 5, lane = lx;
   for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
     const int i = tx * 32 + lx, j = ty * 8 + ly;
@@ -90,6 +91,16 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
       lo_y = __double2float_rd(fmin(fmin(b00y, b10y), fmin(b01y, b11y)));
       hi_y = __double2float_ru(fmax(fmax(b00y, b10y), fmax(b01y, b11y)));
     }
+    // bounding box of the warp's 32 cells (dead lanes carry an empty box: +-1 swapped, widened here to +-inf)
+    float wlo_x = live ? lo_x : INFINITY, whi_x = live ? hi_x : -INFINITY, wlo_y = live ? lo_y : INFINITY,
+          whi_y = live ? hi_y : -INFINITY;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      wlo_x = fminf(wlo_x, __shfl_xor_sync(0xffffffffu, wlo_x, o));
+      whi_x = fmaxf(whi_x, __shfl_xor_sync(0xffffffffu, whi_x, o));
+      wlo_y = fminf(wlo_y, __shfl_xor_sync(0xffffffffu, wlo_y, o));
+      whi_y = fmaxf(whi_y, __shfl_xor_sync(0xffffffffu, whi_y, o));
+    }
     for (int base = 0; base < n_sources; base += LT_SRC_CHUNK) {
       const int cnt = min(LT_SRC_CHUNK, n_sources - base);
       if (n_sources > LT_SRC_CHUNK || tile == (int)blockIdx.x) {      // a single chunk is staged once per CTA
@@ -105,28 +116,23 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
         }
         __syncthreads();
       }
-      // four sources per step: four independent broadcast loads and compare chains, one vote and one (rarely taken)
-      // branch for the group; the padding entries of the last group are boxes no cell can hit
-      for (int k0 = 0; k0 < cnt; k0 += 4) {
-        bool near[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const LtSrcBox b = box[k0 + u];
-          // conservative: P in [lo, hi] in exact arithmetic implies this test passes; one predicate, no short circuit
-          near[u] = (b.x_ru >= lo_x) & (b.x_rd <= hi_x) & (b.y_ru >= lo_y) & (b.y_rd <= hi_y);
-        }
-        if (__any_sync(0xffffffffu, near[0] | near[1] | near[2] | near[3])) {
-#pragma unroll 1
-          for (int u = 0; u < 4; ++u) {
-            if (near[u]) {
-              const int k = k0 + u;
-              const double Px = src[k].x, Py = src[k].y;
-              const int cell = j * nx + i;
-              lt_test_triangle(b00x, b00y, b10x, b10y, b01x, b01y, t1a, t2a, t1b, t2a, t1a, t2b, Px, Py, base + k,
-                               cell, 0, hits, max_hits, n_hits);
-              lt_test_triangle(b11x, b11y, b01x, b01y, b10x, b10y, t1b, t2b, t1a, t2b, t1b, t2a, Px, Py, base + k,
-                               cell, 1, hits, max_hits, n_hits);
-            }
+      // warp-level culling: the 32 cells of a warp (one row segment) share a source-plane bounding box; 32 sources at a
+      // time are tested against it, one per lane, and only the survivors (usually none or one) are tested per cell
+      for (int k0 = 0; k0 < cnt; k0 += 32) {
+        const LtSrcBox bw = box[k0 + lane];        // entries beyond cnt are boxes nothing can hit
+        unsigned m = __ballot_sync(0xffffffffu, (bw.x_ru >= wlo_x) & (bw.x_rd <= whi_x) & (bw.y_ru >= wlo_y) & (bw.y_rd <= whi_y));
+        while (m) {
+          const int k = k0 + __ffs(m) - 1;
+          m &= m - 1;
+          const LtSrcBox b = box[k];
+          // conservative: P in [lo, hi] in exact arithmetic implies this test passes
+          if ((b.x_ru >= lo_x) & (b.x_rd <= hi_x) & (b.y_ru >= lo_y) & (b.y_rd <= hi_y)) {
+            const double Px = src[k].x, Py = src[k].y;
+            const int cell = j * nx + i;
+            lt_test_triangle(b00x, b00y, b10x, b10y, b01x, b01y, t1a, t2a, t1b, t2a, t1a, t2b, Px, Py, base + k, cell,
+                             0, hits, max_hits, n_hits);
+            lt_test_triangle(b11x, b11y, b01x, b01y, b10x, b10y, t1b, t2b, t1a, t2b, t1b, t2a, Px, Py, base + k, cell,
+                             1, hits, max_hits, n_hits);
           }
         }
       }
