@@ -85,11 +85,18 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
       b10x = __dsub_rn(t1b, __dmul_rn(dls_dos, g10.x)); b10y = __dsub_rn(t2a, __dmul_rn(dls_dos, g10.y));
       b01x = __dsub_rn(t1a, __dmul_rn(dls_dos, g01.x)); b01y = __dsub_rn(t2b, __dmul_rn(dls_dos, g01.y));
       b11x = __dsub_rn(t1b, __dmul_rn(dls_dos, g11.x)); b11y = __dsub_rn(t2b, __dmul_rn(dls_dos, g11.y));
-      // conservatively rounded fp32 bounding box: the exact min / max in fp64, then one rounding down / up
-      lo_x = __double2float_rd(fmin(fmin(b00x, b10x), fmin(b01x, b11x)));
-      hi_x = __double2float_ru(fmax(fmax(b00x, b10x), fmax(b01x, b11x)));
-      lo_y = __double2float_rd(fmin(fmin(b00y, b10y), fmin(b01y, b11y)));
-      hi_y = __double2float_ru(fmax(fmax(b00y, b10y), fmax(b01y, b11y)));
+      // conservative fp32 bounding box: corners rounded to nearest (error <= 2^-24 |v|), min / max on the FP32 pipe, then
+      // widened by 2^-23 |v| plus a constant below every coordinate of interest
+      const float f00x = (float)b00x, f10x = (float)b10x, f01x = (float)b01x, f11x = (float)b11x;
+      const float f00y = (float)b00y, f10y = (float)b10y, f01y = (float)b01y, f11y = (float)b11y;
+      lo_x = fminf(fminf(f00x, f10x), fminf(f01x, f11x));
+      hi_x = fmaxf(fmaxf(f00x, f10x), fmaxf(f01x, f11x));
+      lo_y = fminf(fminf(f00y, f10y), fminf(f01y, f11y));
+      hi_y = fmaxf(fmaxf(f00y, f10y), fmaxf(f01y, f11y));
+      lo_x -= fmaf(fabsf(lo_x), 1.1920929e-7f, 1e-30f);
+      hi_x += fmaf(fabsf(hi_x), 1.1920929e-7f, 1e-30f);
+      lo_y -= fmaf(fabsf(lo_y), 1.1920929e-7f, 1e-30f);
+      hi_y += fmaf(fabsf(hi_y), 1.1920929e-7f, 1e-30f);
     }
     // bounding box of the warp's 32 cells (dead lanes carry an empty box: +-1 swapped, widened here to +-inf)
     float wlo_x = live ? lo_x : INFINITY, whi_x = live ? hi_x : -INFINITY, wlo_y = live ? lo_y : INFINITY,
