@@ -95,3 +95,26 @@ def test_argument_errors(env):
     assert e.value.code == -3
     hits, n = lt.lt_find_images(g, 0.0, 0.0, 1.0, 1.0, torch.zeros((0, 2), dtype=torch.float64, device="cuda"))
     assert int(n.item()) == 0
+
+
+def test_round_trip_through_the_lens_equation(env):
+    """The chain of the paper's chi^2 algorithm composed from the library's calls: the predicted images of a source
+    (lt_find_images on the fp64 map of lt_gradient_grid), lensed back with the exact deflection at their positions
+    (lt_gradient_points, eq. 13), land on the source again -- up to the linear-interpolation error of the triangle
+    (second order in the pixel size, larger next to critical lines)."""
+    torch, lt, F = env
+    W = workloads.make(1, paper_regime=True, n_override=801)
+    L = torch.from_numpy(W.lenses).cuda()
+    g = lt.lt_gradient_grid(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, lt.LT_FP64)
+    rng = np.random.default_rng(5)
+    src = rng.uniform(-12, 12, (40, 2))
+    hits, n = lt.lt_find_images(g, W.x_min, W.y_min, W.dx, 1.0, torch.from_numpy(src).cuda())
+    h, n_found = lt.hits_to_numpy(hits, n)
+    assert n_found == len(h) >= 40
+    pos = torch.from_numpy(np.stack([h["x"], h["y"]], axis=1)).cuda()
+    alpha = lt.lt_gradient_points(L, pos).cpu().numpy()
+    beta = np.stack([h["x"], h["y"]], axis=1) - alpha
+    miss = np.hypot(*(beta - src[h["source"]]).T) / W.dx
+    print("round trip: images", len(h), "source-plane miss in pixels: median %.2e, 90%% %.2e, max %.2e" %
+          (np.median(miss), np.quantile(miss, 0.9), miss.max()))
+    assert np.quantile(miss, 0.9) < 0.05 and miss.max() < 1.0
