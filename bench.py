@@ -462,6 +462,32 @@ def run_ours(args, W):
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
                                  "frac": gbs / peaks.get("hbm_gbs", 6650.0),
                                  "algorithmic_bytes": W.nx * W.ny * 16, "peak_source": peak_src}}
+        if rank == 0 and args.mode == "fp64":
+            # the other call of the chi^2 algorithm (step 1): the deflection at a short list of observed image
+            # positions against the whole catalogue -- one warp per point, precompute kernel included
+            import numpy as np
+            pts_fn = {5: lt.lt_gradient_points_sie, 6: lt.lt_gradient_points_nfw}.get(W.lenses.shape[1], lt.lt_gradient_points)
+            rng = np.random.default_rng(W.seed + 78)
+            Ld = torch.from_numpy(W.lenses).cuda()
+            line["points"] = {}
+            for n_pts in (128, 4096):
+                pts = torch.from_numpy(np.stack([rng.uniform(W.x_min, W.x_min + W.dx * (W.nx - 1), n_pts),
+                                                 rng.uniform(W.y_min, W.y_min + W.dx * (W.ny - 1), n_pts)], axis=1)).cuda()
+                po = torch.empty((n_pts, 2), dtype=torch.float64, device="cuda")
+                wsp = lt.alloc_workspace(len(W.lenses), 1, 1, lt.LT_FP64)
+                ts = []
+                for it in range(13):
+                    a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    for _ in range(20):           # back to back: per-call time of a stream of calls
+                        pts_fn(Ld, pts, out=po, workspace=wsp)
+                    b_.record()
+                    torch.cuda.synchronize()
+                    if it >= 3:
+                        ts.append(a.elapsed_time(b_) / 20)
+                us = sum(ts) / len(ts) * 1e3
+                line["points"]["%d_points" % n_pts] = {"us": us, "n_lenses": len(W.lenses),
+                                                       "value": n_pts * len(W.lenses) / (us * 1e-6), "unit": UNIT}
         if rank == 0:
             p64, p32 = lt.lt_peak_probe(0, 1 << 15), lt.lt_peak_probe(1, 1 << 16)
             line["peak_probe"] = {"fp64_tflops": p64 / 1e12, "fp32_tflops": p32 / 1e12,

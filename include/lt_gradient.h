@@ -167,7 +167,12 @@ int lt_gradient_grid_nfw_host(const lt_nfw_lens* h_lenses, int n_lens,
 /*
  * Gradient at an arbitrary list of points (the a9 kernel exposed; used for sampled parity at full size and for
  * image positions).  d_points: n_points*2 doubles (theta_1, theta_2 interleaved); d_out: n_points*2 doubles.
- * fp64 only.  Same workspace rule with nx = ny = 1.
+ * fp64 only.  Same workspace rule with nx = ny = 1.  Lists of more than 4096 points run one thread per point and return,
+ * for a point that is a grid node, the bits of lt_gradient_grid's LT_FP64 map.  Shorter lists (the image positions of
+ * the chi^2 algorithm) run one warp per point, the lenses dealt to the lanes: the same terms, added in another
+ * order, so the result differs from the grid kernel's by the rounding of the sum (a few ulp of the largest term);
+ * it does not depend on the length of the list below that limit.  lt_set_tuning's single_launch bit 2 forces the
+ * thread-per-point kernel for every length.
  */
 int lt_gradient_points(const lt_lens* d_lenses, int n_lens, const double* d_points, long long n_points,
                        double* d_out, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
@@ -224,7 +229,8 @@ int lt_find_images(const double* d_grad, double x_min, double y_min, double dx, 
  * fp64 (1, 2, 4) and fp32 (1, 2, 4) grid kernels; chunk64 / chunk32: lens records staged in shared memory at a time;
  * ctas_per_sm: cap on resident CTAs per SM of the persistent grids; single_launch: bit 0 = one launch of the chosen
  * variant over the whole grid instead of whole waves plus a finer-grained rest, bit 1 = the host
- * entry points always stage the map in device memory and copy it, even into a pinned buffer.  Results do not depend on
+ * entry points always stage the map in device memory and copy it, even into a pinned buffer, bit 2 = lt_gradient_points
+ * runs one thread per point whatever the length of the list.  Results do not depend on
  * any of them except that the fp32 tile centre moves with the pixels per thread of the launch
  * that owns the pixel.  Returns LT_ERR_BAD_SIZE on a negative value.
  */

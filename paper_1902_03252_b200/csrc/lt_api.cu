@@ -25,7 +25,7 @@ namespace {
 thread_local int g_last_cuda_error = 0;
 
 struct Tuning {
-  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0, staged_host_output = 0;
+  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0, staged_host_output = 0, points_per_thread = 0;
 };
 Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
@@ -34,6 +34,7 @@ thread_local int g_launches = 0;                                      // kernels
 constexpr int kDefaultChunk64 = 256;   // 32 KB of fp64 records per CTA
 constexpr int kDefaultChunk32 = 1024;  // 64 KB of fp32 records per CTA
 constexpr size_t kAlign = 256;
+constexpr long long kSplitMaxPoints = 4096;   // lt_gradient_points: lists up to this length run one warp per point (measured crossover ~6000)
 
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
@@ -427,6 +428,19 @@ int gradient_points_impl(const void* d_lenses, int n_lens, const double* d_point
   rc = precompute<M>(d_lenses, n_lens, 1.0, ws, L, st);
   if (rc != LT_OK || n_points == 0) return rc;
   const GridArgs a{n_lens, 0.0, 0.0, 1.0, 1, 1};
+  if (n_points <= kSplitMaxPoints && !g_tuning.points_per_thread) {   /* short list: one warp per point */
+    int grid = 1;
+    constexpr int per_cta = LT_SPLIT_THREADS / 32;
+    rc = grid_for(lt_grad_points_split_kernel<M>, 0, (n_points + per_cta - 1) / per_cta, dev, grid);
+    if (rc != LT_OK) return rc;
+    lt_grad_points_split_kernel<M><<<grid, LT_SPLIT_THREADS, 0, st>>>(
+        reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
+        reinterpret_cast<const LtTables<double>*>(ws + L.tab64), n_lens, reinterpret_cast<const double2*>(d_points),
+        n_points, reinterpret_cast<double2*>(d_out));
+    LT_CUDA(cudaGetLastError());
+    ++g_launches;
+    return LT_OK;
+  }
   return launch_list<M, false>(reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
                             reinterpret_cast<const LtTables<double>*>(ws + L.tab64), a, nullptr,
                             reinterpret_cast<const LtWsHeader*>(ws + L.header),
@@ -524,6 +538,7 @@ int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_s
   if (ppt64 < 0 || ppt32 < 0 || chunk64 < 0 || chunk32 < 0 || ctas_per_sm < 0 || single_launch < 0) return LT_ERR_BAD_SIZE;
   g_tuning.single_launch = single_launch & 1;
   g_tuning.staged_host_output = (single_launch >> 1) & 1;
+  g_tuning.points_per_thread = (single_launch >> 2) & 1;
   g_tuning.ppt64 = ppt64;
   g_tuning.ppt32 = ppt32;
   g_tuning.chunk64 = chunk64;

@@ -308,3 +308,47 @@ lt_grad_list_f64_kernel(const typename M::template Rec<double>::type* __restrict
     lt_list_group<M, FROM_LIST, 1>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
                                 rest0 + g * LT_THREADS, total, out);
 }
+
+// ------------------------------------------------------------------------------------------------ short point lists
+// The observed image positions of the chi^2 algorithm (step 1: "lens the observed images to the source plane"):
+// a few hundred points against the whole catalogue.  One thread per point would leave the machine empty and run the N
+// interactions of a point as one dependent chain, so here a warp owns a point: lane l sums the lenses l, l + 32, ... in
+// catalogue order (two at a time, for two independent chains per lane) and the 32 partial sums are combined by a
+// fixed butterfly.  Every term is the grid kernel's, bit for bit; the order of the sum is not, so the result differs
+// from the grid kernel's by the rounding of the additions only.  The records are read from global memory (L1/L2: the
+// catalogue is a few hundred KB at most), one record per lane.
+#define LT_SPLIT_THREADS 128
+template <class M>
+__global__ void __launch_bounds__(LT_SPLIT_THREADS)
+lt_grad_points_split_kernel(const typename M::template Rec<double>::type* __restrict__ lens,
+                            const LtTables<double>* __restrict__ tables, int n_lens,
+                            const double2* __restrict__ points, long long n_points, double2* __restrict__ out) {
+  typedef typename M::template Rec<double>::type Rec;
+  __shared__ LtTables<double> tab;
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  constexpr int WARPS = LT_SPLIT_THREADS / 32;
+  for (long long p = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5); p < n_points; p += (long long)gridDim.x * WARPS) {
+    const double2 pt = points[p];
+    double A1 = 0.0, A2 = 0.0, B1 = 0.0, B2 = 0.0;
+    int k = lane;
+#pragma unroll 1
+    for (; k + 32 < n_lens; k += 64) {
+      const Rec La = lens[k], Lb = lens[k + 32];
+      M::template interact_sky<double>(pt.x - La.x0, M::template row<double>(pt.y - La.y0, La), La, tab, A1, A2);
+      M::template interact_sky<double>(pt.x - Lb.x0, M::template row<double>(pt.y - Lb.y0, Lb), Lb, tab, B1, B2);
+    }
+    if (k < n_lens) {
+      const Rec La = lens[k];
+      M::template interact_sky<double>(pt.x - La.x0, M::template row<double>(pt.y - La.y0, La), La, tab, A1, A2);
+    }
+    double G1 = __dadd_rn(A1, B1), G2 = __dadd_rn(A2, B2);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      G1 = __dadd_rn(G1, __shfl_xor_sync(0xffffffffu, G1, o));
+      G2 = __dadd_rn(G2, __shfl_xor_sync(0xffffffffu, G2, o));
+    }
+    if (lane == 0) out[p] = make_double2(G1, G2);
+  }
+}

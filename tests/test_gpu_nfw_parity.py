@@ -74,7 +74,7 @@ def test_all_radial_regimes_against_the_quad_oracle(env):
         assert np.abs(g - ref).max() / np.abs(ref).max() < TOL_F64
     W = workloads.make_nfw(n_override=200)
     g64 = _gpu(torch, lt, W, lt.LT_FP64)
-    i, j = rng.integers(0, W.nx, 3000), rng.integers(0, W.ny, 3000)
+    i, j = rng.integers(0, W.nx, 20000), rng.integers(0, W.ny, 20000)      # > 4096: the thread-per-point kernel
     pts = torch.from_numpy(np.stack([W.x_min + i * W.dx, W.y_min + j * W.dx], axis=1)).cuda()
     gp = lt.lt_gradient_points_nfw(torch.from_numpy(W.lenses).cuda(), pts).cpu().numpy()
     assert np.array_equal(gp, g64[j, i])

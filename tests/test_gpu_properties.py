@@ -1,6 +1,7 @@
 """Properties of the CUDA path that hold at any size, for the three lens models (tier 3): superposition
 over lenses (eq. 14-15), permutation of the catalogue, translation of grid and lenses together, a quarter
-turn of the whole configuration.  No oracle involved: the maps are compared with each other."""
+turn of the whole configuration: the maps are compared with each other.  And the short-list kernel of
+lt_gradient_points (one warp per point) against the oracle, the grid kernel and the thread-per-point kernel."""
 import numpy as np
 import pytest
 
@@ -77,3 +78,45 @@ def test_translation_and_quarter_turn(env, model):
     back[..., 0] = rot[:, ::-1, 1].T          # alpha_x(x, y) =  alpha'_y(x', y')
     back[..., 1] = -rot[:, ::-1, 0].T         # alpha_y(x, y) = -alpha'_x(x', y')
     assert np.abs(back - whole).max() / s < 1e-12
+
+
+@pytest.mark.parametrize("model", ["dpie", "sie", "nfw"])
+def test_short_point_lists(env, model):
+    """lt_gradient_points up to 4096 points: one warp per point, lenses dealt to the lanes.  Against the oracle (1e-12),
+    against the thread-per-point kernel and the grid map (same terms, another order of the sum), independent of the
+    length of the list, for catalogue sizes around the lane count (ragged last round, fewer lenses than lanes, none)."""
+    torch, lt = env
+    fn, W, _ = _models(lt)[model]
+    if model == "dpie":
+        from oracle import lt_oracle as Om
+        pts_fn = lt.lt_gradient_points
+    elif model == "sie":
+        from oracle import lt_oracle_sie as Om
+        pts_fn = lt.lt_gradient_points_sie
+    else:
+        from oracle import lt_oracle_nfw as Om
+        pts_fn = lt.lt_gradient_points_nfw
+    rng = np.random.default_rng(8)
+    i, j = rng.integers(0, W.nx, 333), rng.integers(0, W.ny, 333)
+    px, py = W.x_min + i * W.dx, W.y_min + j * W.dx
+    pts = torch.from_numpy(np.stack([px, py], axis=1)).cuda()
+    for n in (len(W.lenses), 65, 64, 33, 31, 1, 0):
+        lenses = np.ascontiguousarray(W.lenses[:n])
+        L = torch.from_numpy(lenses).cuda()
+        short = pts_fn(L, pts).cpu().numpy()
+        if n == 0:
+            assert np.all(short == 0)
+            continue
+        ref = Om.gradient_points(lenses, px, py)
+        s = np.abs(ref).max()
+        assert np.abs(short - ref).max() / s < 1e-12
+        try:
+            lt.lt_set_tuning(single_launch=4)
+            per_thread = pts_fn(L, pts).cpu().numpy()
+        finally:
+            lt.lt_set_tuning()
+        grid = _map(torch, fn, lenses, W)[j, i]
+        assert np.array_equal(per_thread, grid)
+        assert np.abs(short - grid).max() / s < 4e-15
+        assert np.array_equal(pts_fn(L, pts[:100].contiguous()).cpu().numpy(), short[:100])
+        assert np.array_equal(pts_fn(L, pts[:1].contiguous()).cpu().numpy(), short[:1])
