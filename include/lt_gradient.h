@@ -95,6 +95,13 @@ typedef struct {               /* one predicted image found by lt_find_images (3
   double x, y;                 /* image-plane position with the barycentric coordinates of the source point        */
 } lt_image_hit;
 
+typedef struct {               /* written by lt_chi2 (device memory, 32 bytes)                                    */
+  double chi2;                 /* eq. 11 over the observed images that have a predicted counterpart               */
+  long long n_matched;         /* observed images with a term in the sum                                          */
+  long long n_unmatched;       /* observed images whose system has no predicted image (left out of the sum)       */
+  long long reserved;
+} lt_chi2_result;
+
 typedef struct {               /* filled by lt_mixed_last_stats */
   long long n_pixels;          /* -1: not recorded (the caller knows nx*ny)                                      */
   long long n_flagged;         /* pixels recomputed in double precision = patch OR eq.25 OR eq.28                */
@@ -223,6 +230,35 @@ int lt_mixed_rule(const float* d_sp_map, double x_min, double y_min, double dx, 
 int lt_find_images(const double* d_grad, double x_min, double y_min, double dx, int nx, int ny, double dls_dos,
                    const double* d_sources, int n_sources, lt_image_hit* d_hits, int max_hits, int* d_n_hits,
                    void* cuda_stream);
+
+/*
+ * The two small steps that close the chi^2 algorithm around the map (section 2.2.2; eq. 11), so that one
+ * evaluation of the goodness of fit is a sequence of calls on one stream without a host round trip:
+ *   lt_gradient_points (deflection alpha at the observed images) -> lt_source_barycentres -> lt_gradient_grid ->
+ *   lt_find_images (sources = the barycentres) -> lt_chi2.
+ * The observed images of system i are rows d_offsets[i] .. d_offsets[i+1]-1 (n_systems+1 ascending ints, d_offsets[0] = 0,
+ * d_offsets[n_systems] = n_images) of d_theta / d_alpha / d_theta_obs ([n_images, 2] doubles, 16-byte aligned) and of
+ * d_sigma ([n_images] doubles, > 0).  All pointers are device pointers; both calls are asynchronous on cuda_stream.
+ *
+ * lt_source_barycentres: beta_ij = theta_ij - dls_dos * alpha_ij (eq. 13; product and difference rounded
+ * separately), d_barycentres[i] = (sum over j, in catalogue order, of beta_ij) / n_i ([n_systems, 2] doubles); a system
+ * without images gets (nan, nan), which lt_find_images finds in no triangle.  One D_LS/D_OS per call: systems at another
+ * source redshift go through their own sequence of calls.
+ *
+ * lt_chi2: d_terms[j] = |theta_obs_j - x_j|^2 / sigma_j^2 with x_j the predicted image (d_hits / d_n_hits / max_hits as
+ * lt_find_images left them; hit.source = system index) of the image's own system nearest to it -- the paper does not say
+ * how predicted and observed images are paired (reading R28) -- or nan if that system has no predicted image;
+ * d_result->chi2 = the sum of the non-nan terms in catalogue order (eq. 11), with the counts of both kinds.  What a model
+ * that loses images should cost is the caller's decision (R28).  Every operation is a correctly rounded fp64 operation in
+ * the order written here: the result is reproducible bit for bit.
+ * Errors: LT_ERR_BAD_SIZE (negative counts, n_systems > LT_MAX_SOURCES, n_images > 2^24, images without systems),
+ * LT_ERR_NULL_POINTER, LT_ERR_MISALIGNED, LT_ERR_BAD_GRID (dls_dos not finite), LT_ERR_CUDA.
+ */
+int lt_source_barycentres(const double* d_theta, const double* d_alpha, const int* d_offsets, int n_systems,
+                          double dls_dos, double* d_barycentres, void* cuda_stream);
+int lt_chi2(const double* d_theta_obs, const double* d_sigma, const int* d_offsets, int n_systems, int n_images,
+            const lt_image_hit* d_hits, const int* d_n_hits, int max_hits, double* d_terms, lt_chi2_result* d_result,
+            void* cuda_stream);
 
 /*
  * Launch-configuration knobs (process-wide; 0 = the library's default).  ppt64 / ppt32: pixels per thread of the

@@ -10,6 +10,7 @@
 #include "../../include/lt_gradient.h"
 #include "lt_mixed.cuh"
 #include "lt_images.cuh"
+#include "lt_chi2.cuh"
 
 static_assert(sizeof(lt_lens) == sizeof(LtRawLens), "lt_lens and LtRawLens must have the same layout");
 static_assert(sizeof(lt_image_hit) == sizeof(LtImageHit) && sizeof(LtImageHit) == 32, "lt_image_hit layout");
@@ -696,6 +697,52 @@ int lt_find_images(const double* d_grad, double x_min, double y_min, double dx, 
                                                    dls_dos, reinterpret_cast<const double2*>(d_sources), n_sources,
                                                    tiles_x, (int)n_tiles, reinterpret_cast<LtImageHit*>(d_hits), max_hits,
                                                    d_n_hits);
+  LT_CUDA(cudaGetLastError());
+  ++g_launches;
+  return LT_OK;
+}
+
+int lt_source_barycentres(const double* d_theta, const double* d_alpha, const int* d_offsets, int n_systems,
+                          double dls_dos, double* d_barycentres, void* cuda_stream) {
+  if (n_systems < 0 || n_systems > LT_MAX_SOURCES) return LT_ERR_BAD_SIZE;
+  if (n_systems == 0) return LT_OK;
+  if (!d_theta || !d_alpha || !d_offsets || !d_barycentres) return LT_ERR_NULL_POINTER;
+  if (!isfinite(dls_dos)) return LT_ERR_BAD_GRID;
+  if (((uintptr_t)d_theta & 15) || ((uintptr_t)d_alpha & 15) || ((uintptr_t)d_barycentres & 15) || ((uintptr_t)d_offsets & 3))
+    return LT_ERR_MISALIGNED;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  lt_source_barycentres_kernel<<<(n_systems + 127) / 128, 128, 0, st>>>(
+      reinterpret_cast<const double2*>(d_theta), reinterpret_cast<const double2*>(d_alpha), d_offsets, n_systems, dls_dos,
+      reinterpret_cast<double2*>(d_barycentres));
+  LT_CUDA(cudaGetLastError());
+  ++g_launches;
+  return LT_OK;
+}
+
+int lt_chi2(const double* d_theta_obs, const double* d_sigma, const int* d_offsets, int n_systems, int n_images,
+            const lt_image_hit* d_hits, const int* d_n_hits, int max_hits, double* d_terms, lt_chi2_result* d_result,
+            void* cuda_stream) {
+  static_assert(sizeof(lt_chi2_result) == sizeof(LtChi2Result) && sizeof(lt_chi2_result) == 32, "lt_chi2_result layout");
+  if (n_systems < 0 || n_systems > LT_MAX_SOURCES || n_images < 0 || n_images > (1 << 24) || max_hits < 0)
+    return LT_ERR_BAD_SIZE;
+  if (!d_result || !d_n_hits || (max_hits > 0 && !d_hits) ||
+      (n_images > 0 && (!d_theta_obs || !d_sigma || !d_offsets || !d_terms)))
+    return LT_ERR_NULL_POINTER;
+  if (n_images > 0 && n_systems == 0) return LT_ERR_BAD_SIZE;
+  if (((uintptr_t)d_theta_obs & 15) || ((uintptr_t)d_sigma & 7) || ((uintptr_t)d_terms & 7) || ((uintptr_t)d_hits & 7) ||
+      ((uintptr_t)d_result & 7) || ((uintptr_t)d_offsets & 3))
+    return LT_ERR_MISALIGNED;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (n_images > 0) {
+    lt_chi2_terms_kernel<<<(n_images + 127) / 128, 128, 0, st>>>(
+        reinterpret_cast<const double2*>(d_theta_obs), d_sigma, d_offsets, n_systems, n_images,
+        reinterpret_cast<const LtImageHit*>(d_hits), d_n_hits, max_hits, d_terms);
+    LT_CUDA(cudaGetLastError());
+    ++g_launches;
+  }
+  lt_chi2_sum_kernel<<<1, 32, 0, st>>>(d_terms, n_images, reinterpret_cast<LtChi2Result*>(d_result));
   LT_CUDA(cudaGetLastError());
   ++g_launches;
   return LT_OK;

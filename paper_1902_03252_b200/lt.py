@@ -22,6 +22,7 @@ _LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
            "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images", "lt_mixed_rule",
+           "lt_source_barycentres", "lt_chi2",
            "lt_gradient_grid_nfw", "lt_gradient_points_nfw", "lt_gradient_grid_nfw_host",
            "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
 
@@ -83,6 +84,10 @@ def lib():
         L.lt_mixed_rule.restype = ci
         L.lt_find_images.argtypes = [vp, cd, cd, cd, ci, ci, cd, vp, ci, vp, ci, vp, vp]
         L.lt_find_images.restype = ci
+        L.lt_source_barycentres.argtypes = [vp, vp, vp, ci, cd, vp, vp]
+        L.lt_source_barycentres.restype = ci
+        L.lt_chi2.argtypes = [vp, vp, vp, ci, ci, vp, vp, ci, vp, vp, vp]
+        L.lt_chi2.restype = ci
         L.lt_set_tuning.argtypes = [ci, ci, ci, ci, ci, ci]
         L.lt_last_launch_count.restype = ci
         L.lt_set_tuning.restype = ci
@@ -314,6 +319,65 @@ def hits_to_numpy(hits, n_hits):
     n = int(n_hits.item())
     a = hits.cpu().numpy().view(np.dtype(HIT_DTYPE)).reshape(-1)[: min(n, hits.shape[0])]
     return np.sort(a, order=["source", "cell", "triangle"]), n
+
+
+def _offsets_dev(offsets, device):
+    if not (isinstance(offsets, torch.Tensor) and offsets.is_cuda and offsets.dtype == torch.int32):
+        raise TypeError("offsets must be a CUDA int32 tensor [n_systems + 1]")
+    return offsets.contiguous()
+
+
+def lt_source_barycentres(theta, alpha, offsets, dls_dos, out=None, stream=None):
+    """Barycentre, per multiple-image system, of the observed images lensed back into the source plane (eq. 13).
+    theta, alpha: [n_images, 2] float64 CUDA; offsets: [n_systems + 1] int32 CUDA.  Returns [n_systems, 2]."""
+    for t in (theta, alpha):
+        if not (t.is_cuda and t.dtype == torch.float64):
+            raise TypeError("theta and alpha must be CUDA float64 tensors [n_images, 2]")
+    theta, alpha = theta.reshape(-1, 2).contiguous(), alpha.reshape(-1, 2).contiguous()
+    offsets = _offsets_dev(offsets, theta.device)
+    n_sys = offsets.numel() - 1
+    if out is None:
+        out = torch.empty((n_sys, 2), dtype=torch.float64, device=theta.device)
+    rc = lib().lt_source_barycentres(ctypes.c_void_p(theta.data_ptr() if theta.numel() else out.data_ptr()),
+                                     ctypes.c_void_p(alpha.data_ptr() if alpha.numel() else out.data_ptr()),
+                                     ctypes.c_void_p(offsets.data_ptr()), n_sys, float(dls_dos),
+                                     ctypes.c_void_p(out.data_ptr() if n_sys else None), _stream(stream))
+    _check(rc, "lt_source_barycentres")
+    return out
+
+
+def lt_chi2(theta_obs, sigma, offsets, hits, n_hits, terms=None, result=None, stream=None):
+    """Eq. 11 with every observed image paired with the nearest predicted image of its system.  theta_obs [n_images, 2]
+    and sigma [n_images] float64 CUDA, offsets [n_systems + 1] int32 CUDA, hits / n_hits as lt_find_images returned them.
+    Returns (result, terms): a 32-byte uint8 CUDA tensor holding lt_chi2_result (decode with chi2_to_python) and the
+    per-image terms (nan = no predicted image in that system).  Asynchronous."""
+    if not (theta_obs.is_cuda and theta_obs.dtype == torch.float64 and sigma.is_cuda and sigma.dtype == torch.float64):
+        raise TypeError("theta_obs and sigma must be CUDA float64 tensors")
+    theta_obs, sigma = theta_obs.reshape(-1, 2).contiguous(), sigma.reshape(-1).contiguous()
+    n_img = theta_obs.shape[0]
+    if sigma.numel() != n_img:
+        raise ValueError("sigma must have one entry per observed image")
+    offsets = _offsets_dev(offsets, theta_obs.device)
+    n_sys = offsets.numel() - 1
+    if terms is None:
+        terms = torch.empty(max(n_img, 1), dtype=torch.float64, device=theta_obs.device)[:n_img]
+    if result is None:
+        result = torch.empty(32, dtype=torch.uint8, device=theta_obs.device)
+    rc = lib().lt_chi2(ctypes.c_void_p(theta_obs.data_ptr() if n_img else None),
+                       ctypes.c_void_p(sigma.data_ptr() if n_img else None), ctypes.c_void_p(offsets.data_ptr()), n_sys,
+                       n_img, ctypes.c_void_p(hits.data_ptr()), ctypes.c_void_p(n_hits.data_ptr()), int(hits.shape[0]),
+                       ctypes.c_void_p(terms.data_ptr() if n_img else None), ctypes.c_void_p(result.data_ptr()),
+                       _stream(stream))
+    _check(rc, "lt_chi2")
+    return result, terms
+
+
+def chi2_to_python(result):
+    """(synchronises) (chi2, n_matched, n_unmatched) from the 32-byte record lt_chi2 wrote"""
+    import numpy as np
+    raw = result.cpu().numpy().tobytes()
+    return float(np.frombuffer(raw, np.float64, 1)[0]), int(np.frombuffer(raw, np.int64, 3, 8)[0]), \
+        int(np.frombuffer(raw, np.int64, 3, 8)[1])
 
 
 def lt_last_status(workspace, stream=None):

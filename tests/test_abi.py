@@ -76,6 +76,14 @@ def test_argument_errors_need_no_gpu(L):
     assert lib.lt_gradient_grid(vp(16), 4, 0.0, 0.0, 1.0, 8, 8, 2, ctypes.byref(bad), vp(16), vp(16), 1 << 20, None) == -7
     assert lib.lt_gradient_points(vp(16), 4, vp(16), -1, vp(16), vp(16), 1 << 20, None) == -2
     assert lib.lt_set_tuning(-1, 0, 0, 0, 0, 0) == -2 and lib.lt_set_tuning(0, 0, 0, 0, 0, 0) == 0
+    assert lib.lt_source_barycentres(vp(16), vp(16), vp(16), -1, 1.0, vp(16), None) == -2
+    assert lib.lt_source_barycentres(vp(16), None, vp(16), 3, 1.0, vp(16), None) == -1
+    assert lib.lt_source_barycentres(vp(16), vp(24), vp(16), 3, 1.0, vp(16), None) == -6
+    assert lib.lt_source_barycentres(vp(16), vp(16), vp(16), 3, float("inf"), vp(16), None) == -3
+    assert lib.lt_chi2(vp(16), vp(16), vp(16), 2, -1, vp(16), vp(16), 8, vp(16), vp(16), None) == -2
+    assert lib.lt_chi2(vp(16), vp(16), vp(16), 0, 5, vp(16), vp(16), 8, vp(16), vp(16), None) == -2
+    assert lib.lt_chi2(vp(16), vp(16), vp(16), 2, 5, vp(16), vp(16), 8, vp(16), None, None) == -1
+    assert lib.lt_chi2(vp(8), vp(16), vp(16), 2, 5, vp(16), vp(16), 8, vp(16), vp(16), None) == -6
 
 
 def test_binding_refuses_cpu_tensors(L):
