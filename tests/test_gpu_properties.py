@@ -120,3 +120,41 @@ def test_short_point_lists(env, model):
         assert np.abs(short - grid).max() / s < 4e-15
         assert np.array_equal(pts_fn(L, pts[:100].contiguous()).cpu().numpy(), short[:100])
         assert np.array_equal(pts_fn(L, pts[:1].contiguous()).cpu().numpy(), short[:1])
+
+
+def test_two_host_threads_two_streams(env):
+    """The library keeps no per-call state outside the caller's workspace (launch counts and event hooks are per host
+    thread, the occupancy cache is locked): two host threads driving different models and modes on their own streams at
+    the same time get the bits of the serial runs."""
+    import threading
+    torch, lt = env
+    jobs = [(lt.lt_gradient_grid, workloads.make(1, paper_regime=True, n_override=300), lt.LT_MIXED),
+            (lt.lt_gradient_grid_sie, workloads.make_sie("small", n_override=280), lt.LT_FP64),
+            (lt.lt_gradient_grid_nfw, workloads.make_nfw(n_override=260), lt.LT_FP32),
+            (lt.lt_gradient_grid, workloads.make(1, paper_regime=True, n_override=240), lt.LT_FP64)]
+    serial = [_map(torch, fn, W.lenses, W, mode) for fn, W, mode in jobs]
+    results, errors = [None] * len(jobs), []
+
+    def work(k):
+        try:
+            fn, W, mode = jobs[k]
+            st = torch.cuda.Stream()
+            L = torch.from_numpy(np.ascontiguousarray(W.lenses)).cuda()
+            torch.cuda.synchronize()
+            with torch.cuda.stream(st):
+                for _ in range(25):
+                    out = fn(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, stream=st)
+                    n_launch = lt.lt_last_launch_count()
+                    assert n_launch >= 2
+            st.synchronize()
+            results[k] = out.cpu().numpy().astype(np.float64)
+        except Exception as e:  # noqa: BLE001 -- reported by the main thread
+            errors.append((k, repr(e)))
+    threads = [threading.Thread(target=work, args=(k,)) for k in range(len(jobs))]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for k in range(len(jobs)):
+        assert np.array_equal(results[k], serial[k]), k
