@@ -266,7 +266,8 @@ int lt_chi2(const double* d_theta_obs, const double* d_sigma, const int* d_offse
  * ctas_per_sm: cap on resident CTAs per SM of the persistent grids; single_launch: bit 0 = one launch of the chosen
  * variant over the whole grid instead of whole waves plus a finer-grained rest, bit 1 = the host
  * entry points always stage the map in device memory and copy it, even into a pinned buffer, bit 2 = lt_gradient_points
- * runs one thread per point whatever the length of the list.  Results do not depend on
+ * runs one thread per point whatever the length of the list, bit 3 = the grid kernels are launched without the
+ * programmatic-dependent-launch attribute.  Results do not depend on
  * any of them except that the fp32 tile centre moves with the pixels per thread of the launch
  * that owns the pixel.  Returns LT_ERR_BAD_SIZE on a negative value.
  */

@@ -26,7 +26,7 @@ namespace {
 thread_local int g_last_cuda_error = 0;
 
 struct Tuning {
-  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0, staged_host_output = 0, points_per_thread = 0;
+  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0, staged_host_output = 0, points_per_thread = 0, no_dependent_launch = 0;
 };
 Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
@@ -167,6 +167,24 @@ struct KernelEvents {
   }
 };
 
+// Launch of a grid kernel as a programmatic dependent of the kernel before it in the stream (lt_kernels.cuh: the
+// kernel waits for that kernel itself before it reads anything).  lt_set_tuning's single_launch bit 3 switches the
+// attribute off.
+template <class... KArgs, class... Args>
+cudaError_t launch_dependent(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)block);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = g_tuning.no_dependent_launch ? 0 : 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 struct GridArgs {
   int n_lens;
   double x_min, y_min, dx;
@@ -214,9 +232,8 @@ int launch_f64_ppt(const typename Rec64<M>::type* l64, const LtTables<double>* t
   int grid = 1;
   const int rc = grid_for(lt_grad_f64_kernel<M, PPT, MINB>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  lt_grad_f64_kernel<M, PPT, MINB><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
-                                                               a.ny, tiles_x, (int)begin, (int)end, out);
-  LT_CUDA(cudaGetLastError());
+  LT_CUDA(launch_dependent(lt_grad_f64_kernel<M, PPT, MINB>, grid, LT_THREADS, smem, st, l64, t64, a.n_lens, chunk, a.x_min,
+                           a.y_min, a.dx, a.nx, a.ny, tiles_x, (int)begin, (int)end, out));
   ++g_launches;
   return LT_OK;
 }
@@ -247,9 +264,8 @@ int launch_f32_ppt(const typename Rec64<M>::type* l64, const typename Rec32<M>::
   int grid = 1;
   const int rc = grid_for(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
-  lt_grad_f32_kernel<M, PPT, MINB, WIDE><<<grid, LT_THREADS, smem, st>>>(l64, l32, t32, a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx,
-                                                         a.ny, tiles_x, (int)begin, (int)end, out, out_wide);
-  LT_CUDA(cudaGetLastError());
+  LT_CUDA(launch_dependent(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, grid, LT_THREADS, smem, st, l64, l32, t32, a.n_lens, chunk,
+                           a.x_min, a.y_min, a.dx, a.nx, a.ny, tiles_x, (int)begin, (int)end, out, out_wide));
   ++g_launches;
   return LT_OK;
 }
@@ -306,8 +322,9 @@ int check_mixed(const lt_mixed_params& m) {
 template <class M>
 int precompute(const void* d_lenses, int n_lens, double dx, unsigned char* ws, const Layout& L, cudaStream_t st) {
   LT_CUDA(cudaMemsetAsync(ws + L.header, 0, sizeof(LtWsHeader), st));
-  const int blocks = n_lens > 0 ? (n_lens + 127) / 128 : 1;
-  lt_precompute_kernel<M><<<blocks, 128, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, dx,
+  const int blocks = (n_lens > 0 ? (n_lens + LT_PRECOMPUTE_THREADS - 1) / LT_PRECOMPUTE_THREADS : 1) +
+                     (M::kTables ? LT_TABLE_BLOCKS : 0);
+  lt_precompute_kernel<M><<<blocks, LT_PRECOMPUTE_THREADS, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, dx,
                                                reinterpret_cast<typename Rec64<M>::type*>(ws + L.lens64),
                                                reinterpret_cast<typename Rec32<M>::type*>(ws + L.lens32),
                                                reinterpret_cast<LtTables<double>*>(ws + L.tab64),
@@ -540,6 +557,7 @@ int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_s
   g_tuning.single_launch = single_launch & 1;
   g_tuning.staged_host_output = (single_launch >> 1) & 1;
   g_tuning.points_per_thread = (single_launch >> 2) & 1;
+  g_tuning.no_dependent_launch = (single_launch >> 3) & 1;
   g_tuning.ppt64 = ppt64;
   g_tuning.ppt32 = ppt32;
   g_tuning.chunk64 = chunk64;

@@ -16,6 +16,8 @@
 #define LT_WARPS_PER_CTA 8
 #define LT_THREADS (32 * LT_WARPS_PER_CTA)
 #define LT_TILE_H LT_WARPS_PER_CTA
+#define LT_PRECOMPUTE_THREADS 128
+#define LT_TABLE_BLOCKS ((LT_TABLE_ENTRIES + LT_PRECOMPUTE_THREADS - 1) / LT_PRECOMPUTE_THREADS)
 
 struct LtWsHeader {                 // first 256 bytes of the workspace; zeroed at the start of every call
   int bad_code;                     // max over invalid lenses of (n_lens - k); 0 = all valid
@@ -27,6 +29,13 @@ struct LtWsHeader {                 // first 256 bytes of the workspace; zeroed 
 };
 static_assert(sizeof(LtWsHeader) == 256, "workspace header is 256 bytes");
 
+// Programmatic dependent launch (sm_90+): the grid kernels are launched with the programmatic-stream-serialization
+// attribute (lt_api.cu), so their CTAs may be dispatched while the kernel before them in the stream is still running.
+// lt_grid_dependency_wait() returns once that kernel has completed and its writes are visible; lt_launch_dependents()
+// lets the kernel after this one start its dispatch.  Both are no-ops in a launch without the attribute.
+__device__ __forceinline__ void lt_grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void lt_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ------------------------------------------------------------------------------------------------ a1: precompute
 template <class M>
 __global__ void lt_precompute_kernel(const typename M::Raw* __restrict__ raw, int n_lens, double dx,
@@ -34,10 +43,17 @@ __global__ void lt_precompute_kernel(const typename M::Raw* __restrict__ raw, in
                                      typename M::template Rec<float>::type* __restrict__ l32,
                                      LtTables<double>* __restrict__ t64, LtTables<float>* __restrict__ t32,
                                      LtWsHeader* __restrict__ hdr) {
+  // the last LT_TABLE_BLOCKS blocks write the range-reduction tables (lt_math.cuh), one entry per thread, next to the
+  // blocks that pack the lenses: the kernel is one dependent chain per thread, so its duration is the longest chain
+  lt_launch_dependents();
+  const int lens_blocks = (int)gridDim.x - (M::kTables ? LT_TABLE_BLOCKS : 0);
+  if ((int)blockIdx.x >= lens_blocks) {
+    const int e = ((int)blockIdx.x - lens_blocks) * (int)blockDim.x + (int)threadIdx.x;
+    if (e < LT_TABLE_ENTRIES) lt_fill_table_entry(e, *t64, *t32);
+    return;
+  }
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k == 0) hdr->n_lens = n_lens;
-  if (M::kTables && blockIdx.x == gridDim.x - 1)   // the last block also writes the range-reduction tables (lt_math.cuh)
-    for (int e = threadIdx.x; e < LT_TABLE_ENTRIES; e += blockDim.x) lt_fill_table_entry(e, *t64, *t32);
   if (k >= n_lens) return;
   const typename M::Raw r = raw[k];
   typename M::template Rec<double>::type D;
@@ -73,6 +89,7 @@ lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ le
   typedef typename M::template Rec<double>::type Rec;
   __shared__ LtTables<double> tab;
   Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  lt_grid_dependency_wait();
   if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
   __syncthreads();
   constexpr int TILE_W = 32 * PPT;
@@ -139,6 +156,7 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
   typedef typename M::template Rec<double>::type Rec64;
   __shared__ LtTables<float> tab;
   Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  lt_grid_dependency_wait();
   if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));   // visible after the first __syncthreads of the chunk loop
   constexpr int TILE_W = 32 * PPT;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
