@@ -20,6 +20,7 @@ static_assert(sizeof(LtSieLens<double>) == 48 && sizeof(LtSieLens<float>) == 32,
 template <class M> struct Rec64 { typedef typename M::template Rec<double>::type type; };
 template <class M> struct Rec32 { typedef typename M::template Rec<float>::type type; };
 static_assert(sizeof(LtLens<double>) == 128 && sizeof(LtLens<float>) == 64, "lens record sizes");
+static_assert(LT_MAX_LENSES <= LT_BAD_SLOTS * LT_PRECOMPUTE_THREADS, "one bad-code slot per precompute block");
 
 namespace {
 
@@ -40,13 +41,14 @@ constexpr long long kSplitMaxPoints = 4096;   // lt_gradient_points: lists up to
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t header, tab64, tab32, lens64, lens32, flags, sp, list, total;
+  size_t header, bad, tab64, tab32, lens64, lens32, flags, sp, list, total;
 };
 
 Layout make_layout(int n_lens, long long n_pix, bool mixed) {   // dPIE record sizes (the larger) serve both models
   Layout L;
   size_t o = 0;
   L.header = o; o += sizeof(LtWsHeader);
+  L.bad = o;    o += LT_BAD_SLOTS * sizeof(int);   /* directly behind the header: lt_last_status reads both in one copy */
   L.tab64 = o;  o += align_up(sizeof(LtTables<double>));
   L.tab32 = o;  o += align_up(sizeof(LtTables<float>));
   L.lens64 = o; o += align_up((size_t)n_lens * sizeof(LtLens<double>));
@@ -321,7 +323,6 @@ int check_mixed(const lt_mixed_params& m) {
 
 template <class M>
 int precompute(const void* d_lenses, int n_lens, double dx, unsigned char* ws, const Layout& L, cudaStream_t st) {
-  LT_CUDA(cudaMemsetAsync(ws + L.header, 0, sizeof(LtWsHeader), st));
   const int blocks = (n_lens > 0 ? (n_lens + LT_PRECOMPUTE_THREADS - 1) / LT_PRECOMPUTE_THREADS : 1) +
                      (M::kTables ? LT_TABLE_BLOCKS : 0);
   lt_precompute_kernel<M><<<blocks, LT_PRECOMPUTE_THREADS, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, dx,
@@ -329,7 +330,8 @@ int precompute(const void* d_lenses, int n_lens, double dx, unsigned char* ws, c
                                                reinterpret_cast<typename Rec32<M>::type*>(ws + L.lens32),
                                                reinterpret_cast<LtTables<double>*>(ws + L.tab64),
                                                reinterpret_cast<LtTables<float>*>(ws + L.tab32),
-                                               reinterpret_cast<LtWsHeader*>(ws + L.header));
+                                               reinterpret_cast<LtWsHeader*>(ws + L.header),
+                                               reinterpret_cast<int*>(ws + L.bad));
   LT_CUDA(cudaGetLastError());
   ++g_launches;
   return LT_OK;
@@ -768,12 +770,14 @@ int lt_chi2(const double* d_theta_obs, const double* d_sigma, const int* d_offse
 
 int lt_last_status(const void* d_workspace, void* cuda_stream, int* bad_lens_or_null) {
   if (!d_workspace) return LT_ERR_NULL_POINTER;
-  LtWsHeader h;
+  struct { LtWsHeader h; int bad[LT_BAD_SLOTS]; } w;   /* make_layout: the slots follow the header */
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  LT_CUDA(cudaMemcpyAsync(&h, d_workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
+  LT_CUDA(cudaMemcpyAsync(&w, d_workspace, sizeof(w), cudaMemcpyDeviceToHost, st));
   LT_CUDA(cudaStreamSynchronize(st));
-  if (bad_lens_or_null) *bad_lens_or_null = h.bad_code > 0 ? h.n_lens - h.bad_code : -1;
-  return h.bad_code > 0 ? LT_ERR_BAD_LENS_PARAMS : LT_OK;
+  int bad_code = 0;
+  for (int b = 0; b < w.h.bad_blocks && b < LT_BAD_SLOTS; ++b) bad_code = w.bad[b] > bad_code ? w.bad[b] : bad_code;
+  if (bad_lens_or_null) *bad_lens_or_null = bad_code > 0 ? w.h.n_lens - bad_code : -1;
+  return bad_code > 0 ? LT_ERR_BAD_LENS_PARAMS : LT_OK;
 }
 
 int lt_mixed_last_stats(const void* d_workspace, void* cuda_stream, lt_mixed_stats* out) {

@@ -19,8 +19,12 @@
 #define LT_PRECOMPUTE_THREADS 128
 #define LT_TABLE_BLOCKS ((LT_TABLE_ENTRIES + LT_PRECOMPUTE_THREADS - 1) / LT_PRECOMPUTE_THREADS)
 
-struct LtWsHeader {                 // first 256 bytes of the workspace; zeroed at the start of every call
-  int bad_code;                     // max over invalid lenses of (n_lens - k); 0 = all valid
+// Domain check: precompute block b stores max over its invalid lenses of (n_lens - k), 0 = all valid, in slot b of an
+// int array that follows the header (plain stores: nothing has to be zeroed before the kernel runs).
+#define LT_BAD_SLOTS 512            // LT_MAX_LENSES / LT_PRECOMPUTE_THREADS
+
+struct LtWsHeader {                 // first 256 bytes of the workspace; (re)initialised by the precompute kernel
+  int bad_blocks;                   // number of slots of the bad-code array written by this call
   int n_lens;
   unsigned int list_count;          // number of flagged pixels appended to the list (mixed)
   unsigned int pad0;
@@ -42,7 +46,7 @@ __global__ void lt_precompute_kernel(const typename M::Raw* __restrict__ raw, in
                                      typename M::template Rec<double>::type* __restrict__ l64,
                                      typename M::template Rec<float>::type* __restrict__ l32,
                                      LtTables<double>* __restrict__ t64, LtTables<float>* __restrict__ t32,
-                                     LtWsHeader* __restrict__ hdr) {
+                                     LtWsHeader* __restrict__ hdr, int* __restrict__ bad) {
   // the last LT_TABLE_BLOCKS blocks write the range-reduction tables (lt_math.cuh), one entry per thread, next to the
   // blocks that pack the lenses: the kernel is one dependent chain per thread, so its duration is the longest chain
   lt_launch_dependents();
@@ -52,21 +56,34 @@ __global__ void lt_precompute_kernel(const typename M::Raw* __restrict__ raw, in
     if (e < LT_TABLE_ENTRIES) lt_fill_table_entry(e, *t64, *t32);
     return;
   }
+  __shared__ int block_bad;
+  if (threadIdx.x == 0) block_bad = 0;
+  __syncthreads();
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k == 0) hdr->n_lens = n_lens;
-  if (k >= n_lens) return;
-  const typename M::Raw r = raw[k];
-  typename M::template Rec<double>::type D;
-  if (M::valid(r)) {
-    M::pack(r, D);
-  } else {
-    M::poison(D);
-    atomicMax(&hdr->bad_code, n_lens - k);
+  if (k == 0) {                       // the header of this call (the mixed-mode kernels add to the counters later)
+    hdr->bad_blocks = lens_blocks;
+    hdr->n_lens = n_lens;
+    hdr->list_count = 0;
+    hdr->n_patch = 0;
+    hdr->n_eq25 = 0;
+    hdr->n_eq28 = 0;
   }
-  typename M::template Rec<float>::type F;
-  M::round(D, dx, F);
-  l64[k] = D;
-  l32[k] = F;
+  if (k < n_lens) {
+    const typename M::Raw r = raw[k];
+    typename M::template Rec<double>::type D;
+    if (M::valid(r)) {
+      M::pack(r, D);
+    } else {
+      M::poison(D);
+      atomicMax(&block_bad, n_lens - k);
+    }
+    typename M::template Rec<float>::type F;
+    M::round(D, dx, F);
+    l64[k] = D;
+    l32[k] = F;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) bad[blockIdx.x] = block_bad;
 }
 
 // cooperative copy of `count` 16-byte words global -> shared
