@@ -382,6 +382,9 @@ def run_ours(args, W):
                                "MEASURED_PEAKS.json (%s)" % (sms, LANES[mode], sm_max, "64" if LANES[mode] == 64 else "32",
                                                              peak_src),
                 "flops_per_interaction_nominal": r.f_nom, "duration_ms": ms_k,
+                "duration_covers": ("fp64 recompute kernel" if mode == "mixed" else
+                                    "precompute kernel + grid kernels (programmatic dependent launch: an event between "
+                                    "them would serialise them)"),
                 "interactions_per_launch": units, "executed": executed(mode, ms_k, units),
                 "algorithmic_bytes_per_launch": r.out.numel() * r.out.element_size()}
 

@@ -281,7 +281,9 @@ int lt_last_launch_count(void);
  * Measurement hook for bench.py's roofline figure: two cudaEvent_t (as void*; both NULL switches the hook off) that the
  * NEXT calls of lt_gradient_grid on this host thread record on cuda_stream immediately before and after the launch of
  * the dominant kernel (fp64 / fp32 grid kernel; for LT_MIXED the fp64 recompute kernel), so that its duration can be
- * taken on the launching stream without a profiler.  Returns LT_ERR_NULL_POINTER if exactly one is NULL.
+ * taken on the launching stream without a profiler.  In LT_FP64 and LT_FP32 mode the pair also brackets the precompute
+ * kernel (a few microseconds): the grid kernel is launched as its programmatic dependent and an event between the two
+ * would serialise them, so the duration reported is an upper bound of the grid kernels' own.  Returns LT_ERR_NULL_POINTER if exactly one is NULL.
  */
 int lt_set_kernel_events(void* ev_start, void* ev_stop);
 

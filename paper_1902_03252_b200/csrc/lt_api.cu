@@ -241,10 +241,10 @@ int launch_f64_ppt(const typename Rec64<M>::type* l64, const LtTables<double>* t
 }
 template <class M>
 int launch_f64(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
-               const DeviceInfo& d, cudaStream_t st) {
+               const DeviceInfo& d, cudaStream_t st, bool hook = true) {
   // 4 pixels per thread (4 independent chains, lens record loaded once per 4 interactions) at <= 128 registers, two
   // CTAs per SM; fewer pixels per thread for the ragged rest and for grids too small to give every SM two tiles
-  KernelEvents ke(st);
+  KernelEvents ke(st, hook);
   return launch_waves(pick_ppt(g_tuning.ppt64, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
                         switch (ppt) {
@@ -395,10 +395,15 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   const LtTables<float>* t32 = reinterpret_cast<const LtTables<float>*>(ws + L.tab32);
   const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
 
-  rc = precompute<M>(d_lenses, n_lens, dx, ws, L, st);                                   /* a1 */
-  if (rc != LT_OK) return rc;
-  if (mode == LT_FP64) return launch_f64<M>(l64, t64, a, (double2*)d_out_grad, dev, st);      /* a2-a7 */
-  if (mode == LT_FP32) return launch_f32<M>(l64, l32, t32, a, (float2*)d_out_grad, dev, st);
+  {
+    // measurement hook (lt_set_kernel_events): in the fp64 and fp32 modes the pair of events brackets the precompute
+    // kernel too -- the grid kernel is its programmatic dependent, an event between the two would serialise them
+    KernelEvents ke(st, mode != LT_MIXED);
+    rc = precompute<M>(d_lenses, n_lens, dx, ws, L, st);                                   /* a1 */
+    if (rc != LT_OK) return rc;
+    if (mode == LT_FP64) return launch_f64<M>(l64, t64, a, (double2*)d_out_grad, dev, st, /*hook=*/false);   /* a2-a7 */
+    if (mode == LT_FP32) return launch_f32<M>(l64, l32, t32, a, (float2*)d_out_grad, dev, st, /*hook=*/false);
+  }
 
   /* LT_MIXED: single precision everywhere, flag, double precision on the flagged pixels */
   unsigned char* flags = ws + L.flags;
