@@ -306,9 +306,8 @@ int launch_list(const typename Rec64<M>::type* l64, const LtTables<double>* t64,
   const int rc = grid_for(lt_grad_list_f64_kernel<M, FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
   if (rc != LT_OK) return rc;
   KernelEvents ke(st, FROM_LIST);
-  lt_grad_list_f64_kernel<M, FROM_LIST><<<grid, LT_THREADS, smem, st>>>(l64, t64, a.n_lens, chunk, a.x_min, a.y_min, a.dx,
-                                                                    a.nx, list, hdr, points, n_points, out);
-  LT_CUDA(cudaGetLastError());
+  LT_CUDA(launch_dependent(lt_grad_list_f64_kernel<M, FROM_LIST>, grid, LT_THREADS, smem, st, l64, t64, a.n_lens, chunk,
+                           a.x_min, a.y_min, a.dx, a.nx, list, hdr, points, n_points, out));
   ++g_launches;
   return LT_OK;
 }
@@ -395,6 +394,8 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   const LtTables<float>* t32 = reinterpret_cast<const LtTables<float>*>(ws + L.tab32);
   const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
 
+  if (mode == LT_MIXED)   /* the flag map is cleared before the first kernel so that the kernels follow one another */
+    LT_CUDA(cudaMemsetAsync(ws + L.flags, 0, (size_t)n_pix, st));
   {
     // measurement hook (lt_set_kernel_events): in the fp64 and fp32 modes the pair of events brackets the precompute
     // kernel too -- the grid kernel is its programmatic dependent, an event between the two would serialise them
@@ -416,11 +417,9 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   md.h_cluster = mp.patch_halfwidth_cluster;
   md.h_galaxy = mp.patch_halfwidth_galaxy;
   md.b0_cluster = mp.b0_cluster_threshold;
-  LT_CUDA(cudaMemsetAsync(flags, 0, (size_t)n_pix, st));
   if (n_lens > 0) {
-    lt_patch_kernel<M><<<n_lens, 256, 0, st>>>(reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens, x_min, y_min, dx,
-                                            nx, ny, md, flags);
-    LT_CUDA(cudaGetLastError());
+    LT_CUDA(launch_dependent(lt_patch_kernel<M>, n_lens, 256, 0, st, reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens,
+                             x_min, y_min, dx, nx, ny, md, flags));
     ++g_launches;
   }
   rc = launch_f32<M>(l64, l32, t32, a, sp, dev, st, /*hook=*/false, (double2*)d_out_grad);
@@ -429,8 +428,7 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
     long long blocks = (n_pix + 255) / 256;
     const long long cap = (long long)dev.sms * 16;
     if (blocks > cap) blocks = cap;
-    lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(sp, nx, ny, md, flags, list, hdr);   /* a8 */
-    LT_CUDA(cudaGetLastError());
+    LT_CUDA(launch_dependent(lt_flag_kernel, (int)blocks, 256, 0, st, sp, nx, ny, md, flags, list, hdr));   /* a8 */
     ++g_launches;
   }
   return launch_list<M, true>(l64, t64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
@@ -458,11 +456,10 @@ int gradient_points_impl(const void* d_lenses, int n_lens, const double* d_point
     constexpr int per_cta = LT_SPLIT_THREADS / 32;
     rc = grid_for(lt_grad_points_split_kernel<M>, 0, (n_points + per_cta - 1) / per_cta, dev, grid);
     if (rc != LT_OK) return rc;
-    lt_grad_points_split_kernel<M><<<grid, LT_SPLIT_THREADS, 0, st>>>(
-        reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
-        reinterpret_cast<const LtTables<double>*>(ws + L.tab64), n_lens, reinterpret_cast<const double2*>(d_points),
-        n_points, reinterpret_cast<double2*>(d_out));
-    LT_CUDA(cudaGetLastError());
+    LT_CUDA(launch_dependent(lt_grad_points_split_kernel<M>, grid, LT_SPLIT_THREADS, 0, st,
+                             reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
+                             reinterpret_cast<const LtTables<double>*>(ws + L.tab64), n_lens,
+                             reinterpret_cast<const double2*>(d_points), n_points, reinterpret_cast<double2*>(d_out)));
     ++g_launches;
     return LT_OK;
   }

@@ -319,6 +319,7 @@ lt_grad_list_f64_kernel(const typename M::template Rec<double>::type* __restrict
   typedef typename M::template Rec<double>::type Rec;
   __shared__ LtTables<double> tab;
   Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  lt_grid_dependency_wait();
   if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
   __syncthreads();
   const long long total = FROM_LIST ? (long long)hdr->list_count : n_points;
@@ -360,6 +361,7 @@ lt_grad_points_split_kernel(const typename M::template Rec<double>::type* __rest
                             const double2* __restrict__ points, long long n_points, double2* __restrict__ out) {
   typedef typename M::template Rec<double>::type Rec;
   __shared__ LtTables<double> tab;
+  lt_grid_dependency_wait();
   if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
   __syncthreads();
   const int lane = threadIdx.x & 31;

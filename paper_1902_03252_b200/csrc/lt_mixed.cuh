@@ -27,6 +27,7 @@ struct LtMixedDev {          // host-prepared constants of the rule
 template <class M>
 __global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_lens, double x_min, double y_min, double dx,
                                 int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags) {
+  lt_grid_dependency_wait();      // launched as a programmatic dependent (lt_kernels.cuh); keeps the chain of waits whole
   const int k = blockIdx.x;
   if (k >= n_lens) return;
   const double xc = raw[k].x, yc = raw[k].y, b0 = M::patch_scale(raw[k]);   // the lens's deflection scale (R15)
@@ -54,6 +55,7 @@ __global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_l
 __global__ void __launch_bounds__(256)
 lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags,
                unsigned int* __restrict__ list, LtWsHeader* __restrict__ hdr) {
+  lt_grid_dependency_wait();
   const size_t n_pix = (size_t)nx * ny;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   const unsigned lane = threadIdx.x & 31;
