@@ -111,3 +111,11 @@ def test_chain_on_one_stream_against_the_oracle_chain_and_the_sis_closed_form(en
     assert abs(total / total_ref - 1) < 1e-9 and np.abs(terms.cpu().numpy() / terms_ref - 1).max() < 1e-9
     assert abs(total / (12 * delta ** 2 / sigma ** 2) - 1) < 2e-3          # closed form: delta^2 / sigma^2 per image
     print("chi2 chain: gpu %.12g oracle %.12g closed form %.12g" % (total, total_ref, 12 * delta ** 2 / sigma ** 2))
+    # the same on the mixed-precision map (the paper's proposal): the predicted images barely move
+    gm = lt.lt_gradient_grid_sie(L, x_min, x_min, dx, n, n, lt.LT_MIXED)
+    hits_m, n_hits_m = lt.lt_find_images(gm, x_min, x_min, dx, 1.0, bary)
+    res_m, terms_m = lt.lt_chi2(d_obs, d_sig, d_off, hits_m, n_hits_m)
+    total_m, matched_m, unmatched_m = lt.chi2_to_python(res_m)
+    moved = sigma * np.abs(np.sqrt(terms_m.cpu().numpy()) - np.sqrt(terms.cpu().numpy())).max()
+    print("chi2 chain on the mixed map: %.12g, image distances change by at most %.2e arcsec" % (total_m, moved))
+    assert (matched_m, unmatched_m) == (12, 0) and abs(total_m / total - 1) < 1e-3 and moved < 1e-3 * dx
