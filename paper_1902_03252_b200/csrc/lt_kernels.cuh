@@ -141,7 +141,7 @@ lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ le
         const double d2 = t2 - L.y0;                                // Alg. 1 l.4
         const auto row = M::template row<double>(d2, L);            // what the pixels of the row share
 #pragma unroll
-        for (int p = 0; p < PPT; ++p) M::template interact_sky<double>(t1[p] - L.x0, row, L, tab, G1[p], G2[p]);  // l.3, l.5-14
+        for (int p = 0; p < PPT; ++p) M::template interact_sky<double, true>(t1[p] - L.x0, row, L, tab, G1[p], G2[p]);  // l.3, l.5-14
       }
     }
     if (j < ny) {

@@ -159,18 +159,19 @@ struct LtDpieModel {
   static LT_HD void round(const LtLens<double>& D, double dx, LtLens<float>& F) { lt_round_lens(D, dx, F); }
   static LT_HD double patch_scale(const Raw& r) { return r.b0; }
   template <class T> static LT_HD Row<T> row(const T d2, const LtLens<T>& L) { return Row<T>{d2 * L.sx, d2 * L.cy}; }
-  template <class T>
+  // GRID = called from the fp64 grid kernel (lt_sqrt_h: where a hoisted constant pays)
+  template <class T, bool GRID = false>
   static LT_HD void interact_lens(const T X, const T Y, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
     T ax, ay;
-    lt_dpie_body<T>(X, Y, L, tab, ax, ay);
+    lt_dpie_body<T, GRID>(X, Y, L, tab, ax, ay);
     lt_accumulate<T>(ax, ay, L, G1, G2);
   }
-  template <class T>
+  template <class T, bool GRID = false>
   static LT_HD void interact_sky(const T d1, const Row<T>& r, const LtLens<T>& L, const LtTables<T>& tab, T& G1,
                                  T& G2) {
     const T X = lt_fma(d1, L.cx, r.d2sx);            // Alg. 1 l.5, times q/f
     const T Y = lt_fma(-d1, L.sy, r.d2cy);           // Alg. 1 l.6, times 1/f
-    interact_lens<T>(X, Y, L, tab, G1, G2);
+    interact_lens<T, GRID>(X, Y, L, tab, G1, G2);
   }
 };
 struct LtSieModel {
@@ -186,7 +187,7 @@ struct LtSieModel {
   template <class T> static LT_HD LtSieRow<T> row(const T d2, const LtSieLens<T>& L) { return lt_sie_row<T>(d2, L); }
   template <class T>
   static LT_HD void interact_lens(const T, const T, const LtSieLens<T>&, const LtTables<T>&, T&, T&) {}   // unused
-  template <class T>
+  template <class T, bool GRID = false>
   static LT_HD void interact_sky(const T d1, const LtSieRow<T>& r, const LtSieLens<T>& L, const LtTables<T>&, T& G1,
                                  T& G2) {
     lt_sie_interact<T>(d1, r, L, G1, G2);
@@ -207,7 +208,7 @@ struct LtNfwModel {
   }
   template <class T>
   static LT_HD void interact_lens(const T, const T, const LtNfwLens<T>&, const LtTables<T>&, T&, T&) {}   // unused
-  template <class T>
+  template <class T, bool GRID = false>
   static LT_HD void interact_sky(const T d1, const LtSieRow<T>& r, const LtNfwLens<T>& L, const LtTables<T>& tab, T& G1,
                                  T& G2) {
     lt_nfw_interact<T>(d1, r, L, tab, G1, G2);
