@@ -158,3 +158,21 @@ def test_two_host_threads_two_streams(env):
     assert not errors, errors
     for k in range(len(jobs)):
         assert np.array_equal(results[k], serial[k]), k
+
+
+@pytest.mark.parametrize("model", ["dpie", "sie", "nfw"])
+def test_dependent_launch_does_not_change_the_result(env, model):
+    """The grid, patch, flag and list kernels are launched as programmatic dependents of the kernel before them and wait
+    for it before they read anything; with the attribute switched off (lt_set_tuning, bit 3 of
+    single_launch) every mode gives the same bits."""
+    torch, lt = env
+    fn, W, _ = _models(lt)[model]
+    for mode in (0, 1, 2):
+        with_pdl = [_map(torch, fn, W.lenses, W, mode) for _ in range(3)]
+        try:
+            lt.lt_set_tuning(single_launch=8)
+            without = _map(torch, fn, W.lenses, W, mode)
+        finally:
+            lt.lt_set_tuning()
+        for m in with_pdl:
+            assert np.array_equal(m, without), (model, mode)
