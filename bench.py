@@ -56,7 +56,7 @@ PAPER_V100_SIE = {"fp64": 6.9e10, "mixed": 8.2e10}
 LANES = {"fp64": 64, "fp32": 128, "mixed": 64}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at config 1, from the ncu --set full
 # capture summarised in profiles/r01e_ncu_full_summary.md (dPIE kernels at config 1; reads only: the map stays in L2).
-NCU_TRAFFIC_BYTES = {"fp64": 30464, "fp32": 35328, "mixed": 3483648}
+NCU_TRAFFIC_BYTES = {"fp64": 30976, "fp32": 35328, "mixed": 3483648}
 KERNEL_NAME = {"fp64": "lt_grad_f64_kernel", "fp32": "lt_grad_f32_kernel", "mixed": "lt_grad_list_f64_kernel"}
 
 
@@ -358,7 +358,7 @@ def run_ours(args, W):
         if args.model == "nfw":
             return None
         if args.model == "sie":
-            return 6376448 + 664593408 if mode == "fp64" else None
+            return 2343424 + 665636608 if mode == "fp64" else None
         return NCU_TRAFFIC_BYTES[mode] if (args.config == 1 and not args.paper_regime) else None
 
     def executed(mode, ms_k, units):
