@@ -176,9 +176,20 @@ def oracle_module(W):
     return O
 
 
+def host_cores():
+    """Host cores this process may run on.  torch.distributed.run exports OMP_NUM_THREADS=1 to every rank unless the
+    caller has set it, which would time the oracle on one core at N > 1 and on all of them at N = 1: the thread count
+    is therefore passed to the oracle explicitly."""
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except AttributeError:
+        return max(1, os.cpu_count() or 1)
+
+
 def time_oracle(W, stride, threads=0):
     O = oracle_module(W)
     O.lib()
+    threads = threads or host_cores()
     t0 = time.perf_counter()
     O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, precision=O.DOUBLE, n_threads=threads,
                     row_stride=stride)
@@ -191,8 +202,7 @@ def run_reference(args, W):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle import lt_oracle as O0
-    cores = O0.max_threads()
+    cores = host_cores()
     # every step = one bounded sample; the whole run (warmup + steps) is sized to stay within ~2 minutes of wall time
     budget = 100.0 * cores / max(1, args.steps + args.warmup)
     stride, rows = oracle_sample(W, min(args.cpu_seconds, budget))
@@ -558,10 +568,10 @@ def run_ours(args, W):
             line["roofline"]["frac_of_probe"] = line["roofline"]["achieved"] / (
                 (p64 if LANES[args.mode] == 64 else p32) / 1e12)
         if rank == 0 and world == 1:
-            from oracle import lt_oracle as O   # the cpu_baseline leg: the one place bench.py runs the oracle
+            # the cpu_baseline leg: with run_reference the one place bench.py runs the oracle (inside time_oracle)
             stride, rows = oracle_sample(W, args.cpu_seconds)
             v, dt = time_oracle(W, stride)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
                                     "seconds": dt,
                                     "sample": "rows 0,%d,... (%d of %d rows) of %s, `double` instantiation, "
                                               "OpenMP over rows" % (stride, rows, W.ny, W.name)}
