@@ -34,6 +34,13 @@ def test_reference_arm_line(extra, workload):
     assert d["gpu_launches"] == 0 and d["data"] == "synthetic"
 
 
+def test_reference_arm_ignores_the_launchers_omp_default():
+    """torch.distributed.run exports OMP_NUM_THREADS=1 to its ranks; the reference arm must time the oracle on the same
+    cores at every N, so it reports (and uses) the cores of the process, not OpenMP's default."""
+    d = json.loads(_run([], env={"OMP_NUM_THREADS": "1", "RANK": "0", "WORLD_SIZE": "2"}))
+    assert d["cpu_baseline"]["cores"] == len(os.sched_getaffinity(0))
+
+
 def test_reference_arm_other_ranks_are_silent():
     assert _run([], env={"RANK": "1", "WORLD_SIZE": "2"}) == ""
 
