@@ -36,7 +36,9 @@
  * (reading R7); `double` is the timed CPU baseline; `float` is the paper's "identical up to the change in precision"
  * SP version, used for context only; __float128 audits small samples.
  * Known limit: for 1e-14 <= e < 1e-10 the long-double Form C loses ~eps_ld/sqrt(e) relative accuracy (<= 1e-12);
- * no config goes below e = 1e-6.  "parity unpinned" for e >= 0.9 and rcut/rcore -> 1 (outside every config).
+ * no config goes below e = 1e-6.  For e >= 0.9 and rcut/rcore -> 1 (outside every config) the pin is the __float128
+ * instantiation against the density quadrature (tests/test_oracle_pins.py::test_form_q_beyond_the_configs); the long
+ * double one loses rcut/(rcut - rcore) times its rounding there.
  */
 #include <cmath>
 #include <complex>

@@ -59,6 +59,29 @@ def test_form_q_random_tiny():
             assert abs(mp.mpf(float(v[1])) - g2) < tol, (lens, t1, t2)
 
 
+@pytest.mark.parametrize("e,rcore,rcut", [(0.9, 0.3, 12.0), (0.95, 0.5, 30.0), (0.99, 0.2, 8.0), (0.3, 1.0, 1.01),
+                                          (0.6, 2.0, 2.0002), (0.9, 1.0, 1.001)])
+def test_form_q_beyond_the_configs(e, rcore, rcut):
+    """Outside every config (e >= 0.9, rcut/rcore -> 1): the __float128 instantiation, which the GPU test
+    test_fp64_kernel_beyond_the_configs compares with, equals the density quadrature to the rounding of its fp64
+    output; the long double one loses rcut/(rcut - rcore) times its rounding in the difference of the two PIEMD terms."""
+    lens = (0.7, -0.4, e, 0.8, rcore, rcut, 5.0)
+    amp = rcut / (rcut - rcore)
+    for (t1, t2) in [(3.1, 2.2), (0.75, -0.38), (-14.0, 9.0), (0.7 + 1e-3, -0.4 - 2e-3)]:
+        g1, g2 = form_q.gradient_point([lens], t1, t2)
+        s = max(abs(g1), abs(g2))
+        q = O.gradient_points([lens], [t1], [t2], O.QUAD)[0]
+        qn = O.gradient_points([lens], [t1], [t2], O.QUAD, reflect=False)[0]      # as the GPU test calls it
+        v = O.gradient_points([lens], [t1], [t2], O.LONG_DOUBLE)[0]
+        for k, g in ((0, g1), (1, g2)):
+            assert abs(mp.mpf(float(q[k])) - g) / s < 3e-16, (lens, t1, t2, k)
+            assert abs(mp.mpf(float(qn[k])) - g) / s < 3e-16, (lens, t1, t2, k)
+            # long double: relative rounding plus Form C's absolute floor ~ b0/(2 sqrt(e)) eps (see the golden test),
+            # both amplified by rcut/(rcut - rcore)
+            tol = 3e-16 * s + amp * 1.1e-19 * (64 * s + 16 * lens[6] / (2 * np.sqrt(e)))
+            assert abs(mp.mpf(float(v[k])) - g) < tol, (lens, t1, t2, k)
+
+
 def test_reflection_evaluation_matches_unreflected_and_quad():
     """Reading R21: evaluating Form C at (x,-|y|) changes nothing (away from the 0/0 point)."""
     W = workloads.make(0)
