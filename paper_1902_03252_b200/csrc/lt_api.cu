@@ -425,8 +425,8 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   rc = launch_f32<M>(l64, l32, t32, a, sp, dev, st, /*hook=*/false, (double2*)d_out_grad);
   if (rc != LT_OK) return rc;
   {
-    long long blocks = (n_pix + 255) / 256;
-    const long long cap = (long long)dev.sms * 16;
+    long long blocks = (n_pix + LT_FLAG_PPI * 256 - 1) / (LT_FLAG_PPI * 256);
+    const long long cap = (long long)dev.sms * 8;
     if (blocks > cap) blocks = cap;
     LT_CUDA(launch_dependent(lt_flag_kernel, (int)blocks, 256, 0, st, sp, nx, ny, md, flags, list, hdr));   /* a8 */
     ++g_launches;
@@ -683,8 +683,8 @@ int lt_mixed_rule(const float* d_sp_map, double x_min, double y_min, double dx, 
     LT_CUDA(cudaGetLastError());
     ++g_launches;
   }
-  long long blocks = (n_pix + 255) / 256;
-  const long long cap = (long long)dev.sms * 16;
+  long long blocks = (n_pix + LT_FLAG_PPI * 256 - 1) / (LT_FLAG_PPI * 256);
+  const long long cap = (long long)dev.sms * 8;
   if (blocks > cap) blocks = cap;
   lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(reinterpret_cast<const float2*>(d_sp_map), nx, ny, md, d_flags,
                                               reinterpret_cast<unsigned int*>(ws + L.list),

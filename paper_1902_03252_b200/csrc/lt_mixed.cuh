@@ -52,76 +52,107 @@ __global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_l
 // values into the fp64 output, R17),
 // append flagged pixels to the compact list (CTA-aggregated atomic; the order of the list is irrelevant because
 // every pixel is recomputed independently), count.
+// A CTA takes LT_FLAG_PPI * 256 consecutive pixels per iteration, LT_FLAG_PPI per thread (256 apart, so every load is
+// coalesced): the loads of the four pixels and their neighbours are in flight together and the two barriers and the
+// atomic of the append are paid once per 1024 pixels (one pixel per thread: 19 % of the HBM rate at 45 M pixels, bound
+// by load latency and barriers; profiles/r01f_flag_kernel.md).
+#define LT_FLAG_PPI 4
+struct LtFlagLoads { float2 a, bx, by; unsigned char f0; bool fwd_x, fwd_y; };
+// the loads of one pixel, branch-free so that those of the LT_FLAG_PPI pixels of a thread are issued back to back:
+// x neighbour i - 1 (i + 1 at i = 0, R12), y neighbour j - 1 (j + 1 at j = 0); an axis of extent 1 reads the pixel itself
+__device__ __forceinline__ LtFlagLoads lt_flag_load(const float2* __restrict__ sp, unsigned int p, int nx, int ny,
+                                                    const unsigned char* __restrict__ flags) {
+  const unsigned int j = p / (unsigned int)nx, i = p - j * (unsigned int)nx;     // n_pix < 2^32 (the list holds 32-bit indices)
+  LtFlagLoads v;
+  v.fwd_x = i == 0;
+  v.fwd_y = j == 0;
+  const size_t qx = nx > 1 ? (v.fwd_x ? (size_t)p + 1 : (size_t)p - 1) : (size_t)p;
+  const size_t qy = ny > 1 ? (v.fwd_y ? (size_t)p + (size_t)nx : (size_t)p - (size_t)nx) : (size_t)p;
+  v.a = sp[p];
+  v.bx = sp[qx];
+  v.by = sp[qy];
+  v.f0 = flags[p];
+  return v;
+}
+__device__ __forceinline__ unsigned char lt_flag_decide(const LtFlagLoads& v, int nx, int ny, const LtMixedDev& mp) {
+  float c0 = INFINITY, c1 = INFINITY, c2 = 0.f, c3 = 0.f;     // values that never fire
+  if (nx > 1) {                                               // x neighbour: delta_1 (eq. 24), delta_4 (eq. 27)
+    const float d1 = v.fwd_x ? v.bx.x - v.a.x : v.a.x - v.bx.x;
+    const float d4 = v.fwd_x ? v.bx.y - v.a.y : v.a.y - v.bx.y;
+    c0 = fabsf(mp.fdx - d1);
+    c3 = fabsf(d4);
+  }
+  if (ny > 1) {                                               // y neighbour: delta_2 (eq. 24), delta_3 (eq. 27)
+    const float d2 = v.fwd_y ? v.by.y - v.a.y : v.a.y - v.by.y;
+    const float d3 = v.fwd_y ? v.by.x - v.a.x : v.a.x - v.by.x;
+    c1 = fabsf(mp.fdx - d2);
+    c2 = fabsf(d3);
+  }
+  unsigned char f = v.f0 & 1;
+  if (c0 < mp.t25 || c1 < mp.t25) f |= 2;                     // eq. 25
+  if (c2 > mp.t28 || c3 > mp.t28) f |= 4;                     // eq. 28
+  return f;
+}
+
 __global__ void __launch_bounds__(256)
 lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags,
                unsigned int* __restrict__ list, LtWsHeader* __restrict__ hdr) {
   lt_grid_dependency_wait();
   const size_t n_pix = (size_t)nx * ny;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  constexpr size_t TILE = (size_t)LT_FLAG_PPI * 256;
   const unsigned lane = threadIdx.x & 31;
-  unsigned long long c_patch = 0, c25 = 0, c28 = 0;
-  // whole CTAs iterate together (the trip count is rounded up to a multiple of 256 pixels) so that the ballots see a full
-  // mask and the barriers below are reached by every thread
-  __shared__ unsigned int warp_cnt[8], warp_base[8];
   const unsigned wrp = threadIdx.x >> 5;
-  const size_t n_round = (n_pix + 255) / 256 * 256;
-  for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_round; p += stride) {
-    const bool live = p < n_pix;
-    unsigned char f = 0;
-    if (live) {
-      const int j = (int)(p / (size_t)nx), i = (int)(p - (size_t)j * nx);
-      const float2 a = sp[p];
-      float c0 = INFINITY, c1 = INFINITY, c2 = 0.f, c3 = 0.f;     // values that never fire
-      if (nx > 1) {                                               // x neighbour: delta_1 (eq. 24), delta_4 (eq. 27)
-        float d1, d4;
-        if (i > 0) {
-          const float2 b = sp[p - 1];
-          d1 = a.x - b.x;
-          d4 = a.y - b.y;
-        } else {
-          const float2 b = sp[p + 1];
-          d1 = b.x - a.x;
-          d4 = b.y - a.y;
-        }
-        c0 = fabsf(mp.fdx - d1);
-        c3 = fabsf(d4);
-      }
-      if (ny > 1) {                                               // y neighbour: delta_2 (eq. 24), delta_3 (eq. 27)
-        float d2, d3;
-        if (j > 0) {
-          const float2 b = sp[p - nx];
-          d2 = a.y - b.y;
-          d3 = a.x - b.x;
-        } else {
-          const float2 b = sp[p + nx];
-          d2 = b.y - a.y;
-          d3 = b.x - a.x;
-        }
-        c1 = fabsf(mp.fdx - d2);
-        c2 = fabsf(d3);
-      }
-      f = flags[p] & 1;
-      if (c0 < mp.t25 || c1 < mp.t25) f |= 2;                     // eq. 25
-      if (c2 > mp.t28 || c3 > mp.t28) f |= 4;                     // eq. 28
-      flags[p] = f;
-      c_patch += f & 1;
-      c25 += (f >> 1) & 1;
-      c28 += (f >> 2) & 1;
+  unsigned long long c_patch = 0, c25 = 0, c28 = 0;
+  // whole CTAs iterate together so that the ballots see a full mask and the barriers are reached by every thread
+  __shared__ unsigned int seg_base[LT_FLAG_PPI * 8];          // segment s = k * 8 + warp: 32 pixels of sub-tile k
+  for (size_t base = (size_t)blockIdx.x * TILE; base < n_pix; base += (size_t)gridDim.x * TILE) {
+    unsigned char f[LT_FLAG_PPI];
+    unsigned m[LT_FLAG_PPI];
+    LtFlagLoads v[LT_FLAG_PPI];
+#pragma unroll
+    for (int k = 0; k < LT_FLAG_PPI; ++k) {
+      const size_t p = base + (size_t)k * 256 + threadIdx.x;
+      v[k] = lt_flag_load(sp, (unsigned int)(p < n_pix ? p : n_pix - 1), nx, ny, flags);   // past the end: a valid pixel, unused
     }
-    // append: one atomic per CTA and iteration (the eight warps' counts are scanned in shared memory)
-    const unsigned m = __ballot_sync(0xffffffffu, f != 0);
-    if (lane == 0) warp_cnt[wrp] = (unsigned int)__popc(m);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      unsigned int tot = 0;
 #pragma unroll
-      for (int w = 0; w < 8; ++w) { warp_base[w] = tot; tot += warp_cnt[w]; }
-      const unsigned int cta_base = tot ? atomicAdd(&hdr->list_count, tot) : 0u;
+    for (int k = 0; k < LT_FLAG_PPI; ++k) {
+      const size_t p = base + (size_t)k * 256 + threadIdx.x;
+      f[k] = 0;
+      if (p < n_pix) {
+        f[k] = lt_flag_decide(v[k], nx, ny, mp);
+        flags[p] = f[k];
+        c_patch += f[k] & 1;
+        c25 += (f[k] >> 1) & 1;
+        c28 += (f[k] >> 2) & 1;
+      }
+    }
 #pragma unroll
-      for (int w = 0; w < 8; ++w) warp_base[w] += cta_base;
+    for (int k = 0; k < LT_FLAG_PPI; ++k) {
+      m[k] = __ballot_sync(0xffffffffu, f[k] != 0);
+      if (lane == 0) seg_base[k * 8 + wrp] = (unsigned int)__popc(m[k]);
     }
     __syncthreads();
-    if (f != 0) list[warp_base[wrp] + __popc(m & ((1u << lane) - 1u))] = (unsigned int)p;
+    // append: one atomic per CTA and iteration; warp 0 scans the LT_FLAG_PPI * 8 = 32 segment counts
+    if (wrp == 0) {
+      static_assert(LT_FLAG_PPI * 8 == 32, "one segment per lane of warp 0");
+      const unsigned int cnt = seg_base[lane];
+      unsigned int incl = cnt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((int)lane >= o) incl += v;
+      }
+      unsigned int cta_base = 0;
+      if (lane == 31 && incl) cta_base = atomicAdd(&hdr->list_count, incl);
+      cta_base = __shfl_sync(0xffffffffu, cta_base, 31);
+      seg_base[lane] = cta_base + incl - cnt;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < LT_FLAG_PPI; ++k)
+      if (f[k] != 0)
+        list[seg_base[k * 8 + wrp] + __popc(m[k] & ((1u << lane) - 1u))] = (unsigned int)(base + (size_t)k * 256 + threadIdx.x);
+    __syncthreads();                                          // seg_base is rewritten by the next iteration
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
