@@ -418,7 +418,7 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   md.h_galaxy = mp.patch_halfwidth_galaxy;
   md.b0_cluster = mp.b0_cluster_threshold;
   if (n_lens > 0) {
-    LT_CUDA(launch_dependent(lt_patch_kernel<M>, n_lens, 256, 0, st, reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens,
+    LT_CUDA(launch_dependent(lt_patch_kernel<M>, n_lens * LT_PATCH_SPLIT, 256, 0, st, reinterpret_cast<const typename M::Raw*>(d_lenses), n_lens,
                              x_min, y_min, dx, nx, ny, md, flags));
     ++g_launches;
   }
@@ -678,7 +678,7 @@ int lt_mixed_rule(const float* d_sp_map, double x_min, double y_min, double dx, 
   md.h_galaxy = mp.patch_halfwidth_galaxy;
   md.b0_cluster = mp.b0_cluster_threshold;
   if (n_centres > 0) {
-    lt_patch_kernel<LtCentreModel><<<n_centres, 256, 0, st>>>(reinterpret_cast<const LtCentre*>(d_centres), n_centres,
+    lt_patch_kernel<LtCentreModel><<<n_centres * LT_PATCH_SPLIT, 256, 0, st>>>(reinterpret_cast<const LtCentre*>(d_centres), n_centres,
                                                               x_min, y_min, dx, nx, ny, md, d_flags);
     LT_CUDA(cudaGetLastError());
     ++g_launches;

@@ -14,6 +14,7 @@ struct LtCentreModel {
   static __host__ __device__ double patch_scale(const Raw& r) { return r.scale; }
 };
 
+#define LT_PATCH_SPLIT 8
 struct LtMixedDev {          // host-prepared constants of the rule
   float fdx;                 // (float)dx
   float t25;                 // (float)(dx / m_max)
@@ -21,16 +22,25 @@ struct LtMixedDev {          // host-prepared constants of the rule
   double h_cluster, h_galaxy, b0_cluster;
 };
 
-// a8, part 1: one CTA per lens marks its DP patch: the box of half-width hp = max(1, ceil(h/dx)) pixels centred on the
+// a8, part 1: LT_PATCH_SPLIT CTAs per lens mark its DP patch: the box of half-width hp = max(1, ceil(h/dx)) pixels centred on the
 // pixel nearest the lens centre, clipped to the grid (R14); h by lens class (b0 >= threshold: cluster-scale, R15).
 // Overlapping patches write the same value, so plain stores are race-free in effect.
 template <class M>
 __global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_lens, double x_min, double y_min, double dx,
                                 int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags) {
   lt_grid_dependency_wait();      // launched as a programmatic dependent (lt_kernels.cuh); keeps the chain of waits whole
-  const int k = blockIdx.x;
+  const int k = blockIdx.x / LT_PATCH_SPLIT, part = blockIdx.x % LT_PATCH_SPLIT;     // grid: n_lens * LT_PATCH_SPLIT CTAs
   if (k >= n_lens) return;
-  const double xc = raw[k].x, yc = raw[k].y, b0 = M::patch_scale(raw[k]);   // the lens's deflection scale (R15)
+  // one thread reads the lens (the catalogue may sit in pinned host memory: lt_gradient_grid_host), the CTA shares it
+  __shared__ double s_lens[3];
+  if (threadIdx.x == 0) {
+    const typename M::Raw r = raw[k];
+    s_lens[0] = r.x;
+    s_lens[1] = r.y;
+    s_lens[2] = M::patch_scale(r);                                            // the lens's deflection scale (R15)
+  }
+  __syncthreads();
+  const double xc = s_lens[0], yc = s_lens[1], b0 = s_lens[2];
   if (!(isfinite(xc) && isfinite(yc))) return;
   const double h = (b0 >= mp.b0_cluster) ? mp.h_cluster : mp.h_galaxy;
   long long hp = (long long)ceil(h / dx);
@@ -42,7 +52,8 @@ __global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_l
   const long long j0 = max(jc - hp, 0LL), j1 = min(jc + hp, (long long)ny - 1);
   if (i1 < i0 || j1 < j0) return;
   const long long w = i1 - i0 + 1, n = w * (j1 - j0 + 1);
-  for (long long t = threadIdx.x; t < n; t += blockDim.x) {
+  // LT_PATCH_SPLIT CTAs share a lens: a cluster-scale patch is 160 000 pixels at the paper's scale, a galaxy-scale one 441
+  for (long long t = (long long)part * blockDim.x + threadIdx.x; t < n; t += (long long)blockDim.x * LT_PATCH_SPLIT) {
     const long long jj = t / w, ii = t - jj * w;
     flags[(size_t)(j0 + jj) * nx + (size_t)(i0 + ii)] = 1;
   }
