@@ -1,13 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the deflection-map hot path on synthetic cluster catalogues.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--mode fp64|fp32|mixed] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--mode fp64|fp32|mixed] [--shard rows]
+                    [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch: one lt_gradient_grid call (per-lens precompute kernel +
-gradient kernel [+ patch / flag / compaction kernels + fp64 recompute for mixed]) on BASELINE.json config 1
-(1024 x 1024 pixels over [-100,100]", 1 cluster-scale + 99 galaxy-scale dPIE halos, seed 1001; recipe in DESIGN.md
-section 4).  The headline `value` is the fp64 mode (the paper's DP run, Table 2); the same line carries
-the fp32 and mixed numbers on the same workload under "modes".
+gradient kernel [+ patch / flag / compaction kernels + fp64 recompute for mixed]).  The default workload is the LARGEST
+single-GPU configuration of BASELINE.json, config 3 (4096 x 4096 pixels over [-100,100]", 1 cluster-scale + 999
+galaxy-scale dPIE halos, seed 1003, 1.68e10 lens-pixel interactions; recipe in DESIGN.md section 4).  The headline
+`value` is the fp64 mode (the paper's DP run, Table 2); the same line carries
+  * "modes":   fp32 and mixed on the same workload (mixed with its flagged fraction and its time relative to fp64),
+  * "configs": fp64 / fp32 / mixed on BASELINE configs 1, 2, 4 and on the stand-in for the paper's own SIE benchmark
+               (6730 x 6730 pixels, 702 halos; `vs_paper_v100` is context from Table 2, another machine),
+  * "parity":  per mode the error against the long-double CPU oracle on a seeded pixel sample of the SAME workload
+               (20 000 pixels + the pixel nearest every lens centre), with the tolerance it is gated at -- computed in the
+               cpu_baseline leg, outside every timed region (the accuracy the paper asks for: P:280-284),
+  * "roofline", "e2e", "cpu_baseline", "clocks", "gpu_launches" as the contract asks.
 
 Timing: CUDA events on the launching stream around every step, W >= 3 warm-up steps, L2 flushed (a 256 MiB buffer
 is overwritten) between timed steps outside the event pairs, barrier + torch.cuda.synchronize() on both sides of the
@@ -15,15 +23,14 @@ timed region, max over ranks.  `value` has the catalogue already resident in HBM
 lt_gradient_grid_host with pinned HOST buffers (H2D of the catalogue and D2H of the whole map inside the timed region).
 
 N > 1 (torchrun, one rank per GPU): the path shards with no exchange (pixels and MCMC samples are independent,
-P:98): every rank computes the full map of its OWN catalogue (seed + rank) -- weak scaling, no collective
-on the data path; NCCL is used only for the barrier and the max over ranks.
+P:98).  Default: every rank computes the full map of its OWN catalogue (seed + rank) -- weak scaling.
+--shard rows: ONE map cut into contiguous row blocks (paper_1902_03252_b200/shard.py), the catalogue replicated, mixed
+mode with its self-computed halo row -- strong scaling; --gather also times the NCCL all_gather of the blocks.  NCCL is
+otherwise used only for the barrier and the max over ranks.
 
---model sie: the same path with the paper's own lens body (Algorithm 1) on a synthetic stand-in for the paper's benchmark
-(6730 x 6730 pixels at 0.03", 2 cluster-scale + 700 galaxy-scale SIE halos); `vs_baseline` is then the ratio to
-the paper's V100 throughput derived from Table 2 -- another machine's number, context only.
-
---impl reference: times the CPU oracle (oracle/lt_oracle.cpp, `double` instantiation, as it stands) on the host cores,
-each step a bounded row sample of the same workload; rank 0 only.
+--model sie / nfw: the same path with the paper's own lens body (Algorithm 1) on the paper-like benchmark, or with
+pseudo-elliptical NFW halos.  --impl reference: times the CPU oracle (`double` instantiation, as it stands) on the
+host cores, each step a bounded row sample of the same workload; rank 0 only.
 """
 import argparse
 import json
@@ -40,33 +47,38 @@ METRIC = "lens_pixel_gradient_evals_per_s"
 UNIT = "lens*pixel/s"
 MODES = {"fp64": 0, "fp32": 1, "mixed": 2}
 DTYPE = {"fp64": "f64", "fp32": "f32", "mixed": "f32+f64"}
+TOL = {"fp64": 1e-12, "fp32": 1e-5, "mixed": 1e-5}        # DESIGN.md section 7 (of max|alpha| per component)
 
 # FLOP-count convention per lens-pixel interaction (DESIGN.md section 8 / SURVEY 8(d)): textbook evaluation with
 # per-lens constants precomputed, add/sub/mul = 1, FMA = 2: 61 flops + 8 specials (2 sqrt, 2 div, 2 ln, 2 atan2).
-F_NOM = 69.0
-# SIE (Algorithm 1) under the same convention: translate 2 + rotate 6 + R^2 5 + g 4 (with (1 -+ eps) b0
-# precomputed: 2 mul, 2 div by R counted as mul by 1/R) + rotate back 6 + accumulate 2 = 25 flops + 1 rsqrt.
-F_NOM_SIE = 26.0
-# NFW (eq. 16-20 + the circular formula, same convention): translate 2 + rotate 6 + R^2 5 + x 1 + ln(x/2) 1 + F 4 + bracket
-# and scale 3 + eq. 20 8 + rotate back 6 + accumulate 2 = 38 flops + 8 specials (2 sqrt, 3 div, ln, arccosh/arccos, 1/x).
-F_NOM_NFW = 46.0
+F_NOM = {"dpie": 69.0,
+         # SIE (Algorithm 1): translate 2 + rotate 6 + R^2 5 + g 4 + rotate back 6 + accumulate 2 + 1 rsqrt
+         "sie": 26.0,
+         # NFW (eq. 16-20 + the circular formula): 38 flops + 8 specials
+         "nfw": 46.0}
 # the paper's own numbers for the SIE benchmark workload (Table 2 P:364-373 -> BASELINE.md, derived throughput on V100)
 PAPER_V100_SIE = {"fp64": 6.9e10, "mixed": 8.2e10}
 # lanes per SM behind the "alu" peaks (paper's Table 1 convention: 2 ops/cycle x clock x lanes)
 LANES = {"fp64": 64, "fp32": 128, "mixed": 64}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at config 1, from the ncu --set full
-# capture summarised in profiles/r01e_ncu_full_summary.md (dPIE kernels at config 1; reads only: the map stays in L2).
-NCU_TRAFFIC_BYTES = {"fp64": 30976, "fp32": 35328, "mixed": 3483648}
 KERNEL_NAME = {"fp64": "lt_grad_f64_kernel", "fp32": "lt_grad_f32_kernel", "mixed": "lt_grad_list_f64_kernel"}
+# Instructions per interaction of the 4-pixel inner loops, counted in the SASS of the library as built at HEAD
+# (cuobjdump -sass; profiles/README.md says how).  fp64 / mixed: FP64-pipe instructions, each holding an SMSP's 16-lane
+# FP64 pipe for 2 cycles; fp32: all instructions, one issue slot each.
+INSTR_PER_INTERACTION = {("dpie", "fp64"): 61.75, ("dpie", "mixed"): 64.0, ("dpie", "fp32"): 62.75,
+                         ("sie", "fp64"): 12.75, ("sie", "mixed"): 15.75}
+# dram__bytes_{read,write}.sum per launch of the dominant kernels, written by the ncu recipe of profiles/README.md
+NCU_TRAFFIC_JSON = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+MIXED_SIE = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0)   # the paper's rule at its own pixel size; cluster-scale = b0 >= 1"
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1 = the metric's)")
+    ap.add_argument("--config", type=int, default=3,
+                    help="BASELINE.json config index (default 3 = the largest single-GPU configuration)")
     ap.add_argument("--mode", default="fp64", choices=list(MODES))
     ap.add_argument("--paper-regime", action="store_true", help="light galaxy halos (DESIGN.md section 4)")
     ap.add_argument("--m-max", type=float, default=0.0,
@@ -76,7 +88,12 @@ def parse_args():
                     help="dpie: BASELINE.json configs (headline); sie: the paper's Algorithm 1 on its benchmark "
                          "workload, 6730^2 pixels x 702 halos (SURVEY 8(f) NEXT-1); nfw: 2048^2 pixels x 64 "
                          "pseudo-elliptical NFW halos (NEXT-4)")
-    ap.add_argument("--no-extras", action="store_true", help="skip the other modes, cpu_baseline and peak probes")
+    ap.add_argument("--shard", default="none", choices=["none", "rows"],
+                    help="rows: strong scaling, one map cut into row blocks across the ranks (DESIGN.md section 9)")
+    ap.add_argument("--gather", action="store_true", help="with --shard rows: also time the all_gather of the blocks")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="headline only: skip the other modes, configs, parity, cpu_baseline, consumers and peak probes")
+    ap.add_argument("--no-configs", action="store_true", help="skip the `configs` block")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU work of the oracle sample")
     return ap.parse_args()
 
@@ -153,13 +170,26 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-# ------------------------------------------------------------------------------------------------ reference arm
-def oracle_sample(W, cpu_seconds, ns_per_interaction=100.0):
+def ncu_traffic(workload, mode):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the mode's dominant kernel on `workload`, from the
+    ncu --set full capture recorded in profiles/ncu_traffic.json (with the commit it was taken at); None if not captured."""
+    try:
+        rec = json.load(open(NCU_TRAFFIC_JSON))
+        e = rec["captures"]["%s/%s" % (workload, mode)]
+        return {"bytes": e["dram_bytes_read"] + e["dram_bytes_write"], "read": e["dram_bytes_read"],
+                "write": e["dram_bytes_write"], "kernel": e["kernel"], "commit": rec.get("commit")}
+    except Exception:  # noqa: BLE001 -- file absent or workload not captured
+        return None
+
+
+def model_of(W):
+    return {5: "sie", 6: "nfw"}.get(W.lenses.shape[1], "dpie")
+
+
+# ------------------------------------------------------------------------------------------------ reference arm / oracle legs
+def oracle_sample(W, cpu_seconds):
     """Row stride so that the `double` oracle does about `cpu_seconds` of CPU work on this workload."""
-    if W.lenses.shape[1] == 5:
-        ns_per_interaction = 15.0                 # SIE: one sqrt, two divisions
-    if W.lenses.shape[1] == 6:
-        ns_per_interaction = 60.0                 # NFW: log, acosh / acos, two sqrt
+    ns_per_interaction = {"sie": 15.0, "nfw": 60.0, "dpie": 100.0}[model_of(W)]
     total = W.nx * W.ny * len(W.lenses) * ns_per_interaction * 1e-9
     stride = max(1, int(round(total / cpu_seconds)))
     rows = (W.ny + stride - 1) // stride
@@ -167,9 +197,9 @@ def oracle_sample(W, cpu_seconds, ns_per_interaction=100.0):
 
 
 def oracle_module(W):
-    if W.lenses.shape[1] == 6:
+    if model_of(W) == "nfw":
         from oracle import lt_oracle_nfw as O
-    elif W.lenses.shape[1] == 5:
+    elif model_of(W) == "sie":
         from oracle import lt_oracle_sie as O
     else:
         from oracle import lt_oracle as O
@@ -228,44 +258,100 @@ def run_reference(args, W):
     print(json.dumps(line), flush=True)
 
 
+def parity_sample(W, n_random=20000):
+    """Seeded pixel sample of a workload: n_random pixels drawn uniformly plus the pixel nearest every lens centre that
+    lies inside the grid.  Returns (i, j) int64 arrays.  No arithmetic of the method: indices only."""
+    import numpy as np
+    rng = np.random.default_rng(W.seed + 4242)
+    i = rng.integers(0, W.nx, n_random)
+    j = rng.integers(0, W.ny, n_random)
+    ic = np.rint((W.lenses[:, 0] - W.x_min) / W.dx).astype(np.int64)
+    jc = np.rint((W.lenses[:, 1] - W.y_min) / W.dx).astype(np.int64)
+    ok = (ic >= 0) & (ic < W.nx) & (jc >= 0) & (jc < W.ny)
+    return np.concatenate([i, ic[ok]]), np.concatenate([j, jc[ok]])
+
+
+def oracle_parity(W, sampled, flags_sampled, mixed_params):
+    """The cpu_baseline leg's second job (the one other place this file runs the oracle): the long-double oracle at the
+    sampled pixels against what each mode's map holds there.  `sampled`: {mode: float64 array [n, 2]} gathered from the
+    GPU maps outside the timed regions.  Metric of DESIGN.md reading R9: per component, max |GPU - oracle| / max |oracle|."""
+    import numpy as np
+    O = oracle_module(W)
+    i, j = parity_sample(W)
+    px = W.x_min + i.astype(np.float64) * W.dx           # fl(x_min + fl(i dx)): the coordinates the API defines
+    py = W.y_min + j.astype(np.float64) * W.dx
+    ref = O.gradient_points(W.lenses, px, py, n_threads=host_cores())
+    scale = np.abs(ref).max(axis=0)
+    out = {}
+    sie = model_of(W) == "sie"
+    in_patch = (flags_sampled & 1) != 0 if flags_sampled is not None else np.zeros(len(i), bool)
+    for mode, got in sampled.items():
+        err = np.abs(got - ref) / scale
+        gate = np.ones(len(i), bool)
+        if sie and mode == "fp32":
+            gate = ~in_patch          # R10: fp32 is gated outside the rule's DP patches, reported inside (A.65, P:876-880)
+        e = {"max_err_rel": float(err[gate].max()), "rms_err_rel": float(np.sqrt((err[gate] ** 2).mean())),
+             "tol": TOL[mode], "n_sampled": int(gate.sum()), "pass": bool(err[gate].max() < TOL[mode])}
+        if sie and mode == "fp32" and in_patch.any():
+            e["max_err_rel_inside_dp_patches_reported_not_gated"] = float(err[in_patch].max())
+        if mode == "mixed" and flags_sampled is not None:
+            fl = flags_sampled != 0
+            e["n_flagged_in_sample"] = int(fl.sum())
+            if "fp64" in sampled:
+                e["flagged_bit_equal_to_fp64_mode"] = bool(np.array_equal(got[fl], sampled["fp64"][fl]))
+            e["paper_criterion_dx_over_4M"] = {"m_max": mixed_params[0], "bound_arcsec": W.dx / 4.0 / mixed_params[0],
+                                               "max_abs_err_unflagged_arcsec":
+                                                   float(np.abs(got - ref)[~fl].max()) if (~fl).any() else 0.0}
+        out[mode] = e
+    out["_sample"] = "%d seeded pixels + %d lens-centre pixels of %s; oracle = long double Form C" % (
+        20000, len(i) - 20000, W.name)
+    return out
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 class Runner:
-    """Holds the device buffers of one workload/mode and issues steps through the C ABI (python = marshalling)."""
+    """Holds the device buffers of one workload/mode and issues steps through the C ABI (python = marshalling).
+    `block`: a shard.RowBlock -- the rows of the global map this rank computes (--shard rows)."""
 
-    def __init__(self, torch, lt, W, mode):
+    def __init__(self, torch, lt, W, mode, m_max=0.0, block=None, host=True):
         self.torch, self.lt, self.W, self.mode = torch, lt, W, mode
         self.code = MODES[mode]
         n = len(W.lenses)
-        self.sie = W.lenses.shape[1] == 5
-        self.nfw = W.lenses.shape[1] == 6
-        self.grid = {5: lt.lt_gradient_grid_sie, 6: lt.lt_gradient_grid_nfw}.get(W.lenses.shape[1], lt.lt_gradient_grid)
-        self.grid_host = {5: lt.lt_gradient_grid_sie_host, 6: lt.lt_gradient_grid_nfw_host}.get(W.lenses.shape[1],
-                                                                                                lt.lt_gradient_grid_host)
-        # SIE: the paper's rule at its own pixel size; cluster-scale = b0 >= 1" (its cluster halos: 28.8", 14.1")
-        self.mixed = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0) if self.sie else None
-        if M_MAX > 0:
-            self.mixed = (M_MAX, 0.5 * (1.0 - 1.0 / M_MAX), 0.0, 0.0, 1e300)
+        self.model = model_of(W)
+        cols = W.lenses.shape[1]
+        self.grid = {5: lt.lt_gradient_grid_sie, 6: lt.lt_gradient_grid_nfw}.get(cols, lt.lt_gradient_grid)
+        self.grid_host = {5: lt.lt_gradient_grid_sie_host, 6: lt.lt_gradient_grid_nfw_host}.get(cols, lt.lt_gradient_grid_host)
+        self.mixed = MIXED_SIE if self.model == "sie" else None
+        if m_max > 0:
+            self.mixed = (m_max, 0.5 * (1.0 - 1.0 / m_max), 0.0, 0.0, 1e300)
+        self.mixed_params = self.mixed or (3.26, 0.0104 / 0.03, 6.0, 0.3, 15.0)
+        self.y_min, self.ny, self.halo = W.y_min, W.ny, 0
+        if block is not None:
+            self.y_min, self.ny, self.halo = block.y_min, block.ny, block.halo
         self.d_lenses = torch.from_numpy(W.lenses).cuda()
         dt = torch.float32 if mode == "fp32" else torch.float64
-        self.out = torch.empty((W.ny, W.nx, 2), dtype=dt, device="cuda")
-        self.ws = lt.alloc_workspace(n, W.nx, W.ny, self.code)
-        self.h_lenses = torch.from_numpy(W.lenses).pin_memory()
-        self.h_out = torch.empty((W.ny, W.nx, 2), dtype=dt).pin_memory()
-        self.ws_host = lt.alloc_workspace(n, W.nx, W.ny, self.code, host=True)
-        self.units = W.nx * W.ny * n
-        self.h2d = self.h_lenses.numel() * 8
-        self.f_nom = F_NOM_SIE if self.sie else (F_NOM_NFW if self.nfw else F_NOM)
-        self.d2h = self.h_out.numel() * self.h_out.element_size()
+        self.out = torch.empty((self.ny, W.nx, 2), dtype=dt, device="cuda")
+        self.ws = lt.alloc_workspace(n, W.nx, self.ny, self.code)
+        self.units = W.nx * W.ny * n                      # of the WHOLE map (a row block's share is added up by the caller)
+        self.units_local = W.nx * (self.ny - self.halo) * n
+        self.f_nom = F_NOM[self.model]
+        self.launches = 0
+        if host:
+            self.h_lenses = torch.from_numpy(W.lenses).pin_memory()
+            self.h_out = torch.empty((self.ny, W.nx, 2), dtype=dt).pin_memory()
+            self.ws_host = lt.alloc_workspace(n, W.nx, self.ny, self.code, host=True)
+            self.h2d = self.h_lenses.numel() * 8
+            self.d2h = self.h_out.numel() * self.h_out.element_size()
 
     def step(self):
         W = self.W
-        self.grid(self.d_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, mixed=self.mixed, out=self.out,
+        self.grid(self.d_lenses, W.x_min, self.y_min, W.dx, W.nx, self.ny, self.code, mixed=self.mixed, out=self.out,
                   workspace=self.ws)
         self.launches = self.lt.lt_last_launch_count()      # kernels of ours this step enqueued (memsets not counted)
 
     def step_host(self):
         W = self.W
-        self.grid_host(self.h_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, self.code, self.h_out, self.ws_host,
+        self.grid_host(self.h_lenses, W.x_min, self.y_min, W.dx, W.nx, self.ny, self.code, self.h_out, self.ws_host,
                        mixed=self.mixed)
 
 
@@ -273,7 +359,7 @@ def timed(torch, lt, fn, steps, warmup, flush, barrier):
     """W warm-up steps, then K steps each bracketed by CUDA events on the current stream; L2 flushed between steps
     (outside the event pairs).  A second event pair per step, recorded by the library itself around the dominant
     kernel's launch (lt_set_kernel_events), gives that kernel's duration inside the same timed region.
-    Returns (mean step time [ms], mean dominant-kernel time [ms])."""
+    Returns (mean step time [ms], mean dominant-kernel time [ms], spread)."""
     for _ in range(warmup):
         fn()
         flush.fill_(1)
@@ -299,141 +385,347 @@ def timed(torch, lt, fn, steps, warmup, flush, barrier):
     torch.cuda.synchronize()
     lt.lt_set_kernel_events(None, None)
     per_step = sorted(a.elapsed_time(b) for a, b in ev)
-    timed.last_spread = {"median": per_step[len(per_step) // 2], "best": per_step[0], "worst": per_step[-1]}
-    return sum(per_step) / steps, sum(a.elapsed_time(b) for a, b in kev) / steps
+    spread = {"median": per_step[len(per_step) // 2], "best": per_step[0], "worst": per_step[-1]}
+    return sum(per_step) / steps, sum(a.elapsed_time(b) for a, b in kev) / steps, spread
 
 
-def run_ours(args, W):
-    import torch
-    from paper_1902_03252_b200 import lt
-    lt.lib()                                          # raises if the CUDA library is missing: no fallback
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference)")
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-        from paper_1902_03252_b200 import workloads
-        W = make_workload(args, seed_offset=rank)                                           # own catalogue per rank
+class Bench:
+    """One process = one rank; holds what every measurement shares."""
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
+    def __init__(self, args):
+        import torch
+        from paper_1902_03252_b200 import lt
+        lt.lib()                                          # raises if the CUDA library is missing: no fallback
+        if not torch.cuda.is_available():
+            raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference)")
+        self.torch, self.lt, self.args = torch, lt, args
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        torch.cuda.set_device(self.local)
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+            self.dist = dist
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        self.peaks, self.peak_src = measured_peaks()
+        self.sms = torch.cuda.get_device_properties(self.local).multi_processor_count
+        self.sm_max = float(self.peaks.get("sm_max_mhz") or 1965.0)
+        self.sm_run = self.sm_max
 
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    peaks, peak_src = measured_peaks()
-    sms = torch.cuda.get_device_properties(local).multi_processor_count
-    sampler = ClockSampler(physical_index(local))
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
 
-    def measure(mode, steps, warmup, host=False):
-        r = Runner(torch, lt, W, mode)
+    def max_over_ranks(self, ms):
+        if self.dist is None:
+            return ms
+        t = self.torch.tensor([ms], dtype=self.torch.float64, device="cuda")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def measure(self, W, mode, steps, warmup, host=False, block=None):
+        """-> dict(ms, ms_kernel, spread, extra, runner); ms = max over ranks of the mean step time"""
+        lt = self.lt
+        r = Runner(self.torch, lt, W, mode, m_max=self.args.m_max, block=block, host=host)
         fn = r.step_host if host else r.step
-        ms, ms_kernel = timed(torch, lt, fn, steps, warmup, flush, barrier)
-        rc, bad = lt.lt_last_status(r.ws_host if host else r.ws)
+        ms, ms_kernel, spread = timed(self.torch, lt, fn, steps, warmup, self.flush, self.barrier)
+        ws = r.ws_host if host else r.ws
+        rc, bad = lt.lt_last_status(ws)
         if rc != 0:
             raise RuntimeError("lens parameter domain error at lens %d" % bad)
-        r.ms_kernel = ms_kernel
-        if dist is not None:
-            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms_local = ms
+        ms = self.max_over_ranks(ms)
         extra = {}
         if mode == "mixed":
-            st = lt.lt_mixed_last_stats(r.ws_host if host else r.ws)
-            extra = {"flagged_fraction": st["n_flagged"] / (W.nx * W.ny), "patch_fraction": st["n_patch"] / (W.nx * W.ny),
-                     "eq25_fraction": st["n_eq25"] / (W.nx * W.ny), "eq28_fraction": st["n_eq28"] / (W.nx * W.ny)}
-        return r, ms, extra
+            st = lt.lt_mixed_last_stats(ws)
+            n_pix = W.nx * r.ny
+            extra = {"flagged_fraction": st["n_flagged"] / n_pix, "patch_fraction": st["n_patch"] / n_pix,
+                     "eq25_fraction": st["n_eq25"] / n_pix, "eq28_fraction": st["n_eq28"] / n_pix}
+        return {"ms": ms, "ms_local": ms_local, "ms_kernel": ms_kernel, "spread": spread, "extra": extra, "runner": r}
 
-    # ---- headline: the requested mode, device-resident inputs
-    sampler.start()
-    r, ms, extra = measure(args.mode, args.steps, args.warmup)
-    spread = dict(timed.last_spread)             # this rank's timed steps (median and best beside the mean)
-    value = world * r.units / (ms * 1e-3)
-    # ---- e2e: same metric through the host-buffer entry point
-    e2e_steps = max(3, min(args.steps, 50))
-    _, ms_e2e, _ = measure(args.mode, e2e_steps, max(3, min(args.warmup, 5)), host=True)
-    clocks = sampler.stop()
-
-    ms_kernel_main = r.ms_kernel        # dominant kernel, events recorded by the library inside the timed steps
-    sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0)
-    sm_run = float(clocks.get("sm_mhz") or sm_max)        # median SM clock sampled during the timed region
-
-    def traffic(mode):
-        # per launch of the dominant kernel, from the ncu --set full captures under profiles/ (None where not captured)
-        if args.model == "nfw":
-            return None
-        if args.model == "sie":
-            return 2343424 + 665636608 if mode == "fp64" else None
-        return NCU_TRAFFIC_BYTES[mode] if (args.config == 1 and not args.paper_regime) else None
-
-    def executed(mode, ms_k, units):
-        """The same launch against the instruction floor of the pipe that bounds it: instructions per interaction counted
-        in the SASS of the 4-pixel inner loop (profiles/r01e_ncu_full_summary.md).  fp64 / mixed: FP64-pipe instructions,
-        each holding an SMSP's 16-lane FP64 pipe for 2 cycles; fp32: all instructions, one issue slot each."""
-        per = {("dpie", "fp64"): 61.75, ("dpie", "mixed"): 61.75, ("dpie", "fp32"): 62.75,
-               ("sie", "fp64"): 12.75, ("sie", "mixed"): 12.75, ("sie", "fp32"): None}.get((args.model, mode))
+    # ---- roofline of one measurement
+    def executed(self, model, mode, ms_k, units):
+        """The same launch against the instruction floor of the pipe that bounds it."""
+        per = INSTR_PER_INTERACTION.get((model, mode))
         if per is None:
             return None
         cycles = per * (2.0 if mode != "fp32" else 1.0)
-        floor = sms * 4 * sm_max * 1e6 * 32 / cycles                   # interactions per second at 100 % of the pipe
-        return {"instructions_per_interaction": per, "pipe": "fp64 (2 cycles per warp instruction)" if mode != "fp32"
-                else "issue slots (1 per warp instruction)", "floor_interactions_per_s": floor,
-                "frac_of_floor": units / (ms_k * 1e-3) / floor}
+        floor = self.sms * 4 * self.sm_max * 1e6 * 32 / cycles          # interactions per second at 100 % of the pipe
+        return {"instructions_per_interaction": per,
+                "pipe": "fp64 (2 cycles per warp instruction)" if mode != "fp32" else "issue slots (1 per warp instruction)",
+                "floor_interactions_per_s": floor, "frac_of_floor": units / (ms_k * 1e-3) / floor}
 
-    def roofline(mode, ms_k, units, flagged=1.0):
+    def roofline(self, W, m, mode):
+        r = m["runner"]
         # mixed: the dominant kernel is the fp64 recompute, which processes the flagged pixels only
-        units = units * flagged
-        peak = 2.0 * sms * LANES[mode] * sm_max * 1e6 / 1e12
+        units = r.units_local * m["extra"].get("flagged_fraction", 1.0)
+        ms_k = m["ms_kernel"]
+        peak = 2.0 * self.sms * LANES[mode] * self.sm_max * 1e6 / 1e12
         ach = r.f_nom * units / (ms_k * 1e-3) / 1e12
+        tr = ncu_traffic(W.name, mode)
         return {"bound": "alu", "kernel": KERNEL_NAME[mode], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "frac_at_sampled_clock": ach / (peak * sm_run / sm_max), "traffic": traffic(mode),
+                "frac": ach / peak, "frac_at_sampled_clock": ach / (peak * self.sm_run / self.sm_max),
+                "traffic": tr["bytes"] if tr else None, "traffic_source": tr,
                 "peak_source": "derived: 2 x %d SMs x %d lanes x %.0f MHz (DESIGN.md section 8); no FP%s vector peak in "
-                               "MEASURED_PEAKS.json (%s)" % (sms, LANES[mode], sm_max, "64" if LANES[mode] == 64 else "32",
-                                                             peak_src),
+                               "MEASURED_PEAKS.json (%s)" % (self.sms, LANES[mode], self.sm_max,
+                                                             "64" if LANES[mode] == 64 else "32", self.peak_src),
                 "flops_per_interaction_nominal": r.f_nom, "duration_ms": ms_k,
                 "duration_covers": ("fp64 recompute kernel" if mode == "mixed" else
                                     "precompute kernel + grid kernels (programmatic dependent launch: an event between "
                                     "them would serialise them)"),
-                "interactions_per_launch": units, "executed": executed(mode, ms_k, units),
+                "interactions_per_launch": units, "executed": self.executed(r.model, mode, ms_k, units),
                 "algorithmic_bytes_per_launch": r.out.numel() * r.out.element_size()}
 
+    # ---- the three modes of one workload, briefly (the `configs` block)
+    def three_modes(self, W, steps, warmup):
+        out = {"n_lens": int(len(W.lenses)), "nx": W.nx, "ny": W.ny, "interactions": W.nx * W.ny * len(W.lenses)}
+        sampled, flags_s, mp = {}, None, None
+        for mode in MODES:
+            m = self.measure(W, mode, steps, warmup)
+            r = m["runner"]
+            e = {"value": r.units / (m["ms"] * 1e-3), "ms_per_step": m["ms"], "kernel_ms": m["ms_kernel"],
+                 "roofline_frac_nominal": self.roofline(W, m, mode)["frac"], **m["extra"]}
+            ex = self.executed(r.model, mode, m["ms_kernel"], r.units_local * m["extra"].get("flagged_fraction", 1.0))
+            if ex:
+                e["frac_of_floor"] = ex["frac_of_floor"]
+            if r.model == "sie" and mode in PAPER_V100_SIE:
+                e["vs_paper_v100"] = e["value"] / PAPER_V100_SIE[mode]
+            out[mode] = e
+            s, f = self.sample_map(W, r)
+            sampled[mode] = s
+            if f is not None:
+                flags_s, mp = f, r.mixed_params
+            del m, r
+        out["mixed"]["time_vs_fp64"] = out["mixed"]["ms_per_step"] / out["fp64"]["ms_per_step"]
+        return out, sampled, flags_s, mp
+
+    def sample_map(self, W, r):
+        """What the runner's last map holds at the seeded sample pixels (float64 numpy [n, 2]); for mixed also the flags."""
+        torch = self.torch
+        i, j = parity_sample(W)
+        idx = torch.from_numpy(j * W.nx + i).cuda()
+        got = r.out.reshape(-1, 2)[idx].double().cpu().numpy()
+        flags = None
+        if r.mode == "mixed":
+            f = self.lt.lt_mixed_last_flags(r.ws, len(W.lenses), W.nx, W.ny)
+            flags = f.reshape(-1)[idx].cpu().numpy()
+        return got, flags
+
+
+def consumers(B, W, r, line):
+    """The consumers of the map (section 2.2.2) on the fp64 map just computed: triangle search, gradient at image
+    positions, one whole chi^2 evaluation on one stream.  Rank 0, fp64 headline only."""
+    import numpy as np
+    torch, lt, flush = B.torch, B.lt, B.flush
+    rng = np.random.default_rng(W.seed + 77)
+    src_all = torch.from_numpy(rng.normal(0.0, 8.0, (64, 2)) + W.lenses[0, :2]).cuda()
+    hits = torch.empty((1 << 16, 32), dtype=torch.uint8, device="cuda")
+    n_hits = torch.empty(1, dtype=torch.int32, device="cuda")
+    line["find_images"] = {}
+    for n_src in (4, 64):                 # few sources: bound by reading the map; many: by the source loop
+        src = src_all[:n_src].contiguous()
+        ts = []
+        for it in range(8):
+            flush.fill_(1)
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            lt.lt_find_images(r.out, W.x_min, W.y_min, W.dx, 1.0, src, hits=hits, n_hits=n_hits)
+            b_.record()
+            torch.cuda.synchronize()
+            if it >= 3:
+                ts.append(a.elapsed_time(b_))
+        ms_fi = sum(ts) / len(ts)
+        gbs = W.nx * W.ny * 16 / (ms_fi * 1e-3) / 1e9
+        line["find_images"]["%d_sources" % n_src] = {
+            "ms": ms_fi, "images_found": int(n_hits.item()),
+            "cells_per_s": (W.nx - 1) * (W.ny - 1) / (ms_fi * 1e-3),
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": B.peaks.get("hbm_gbs"), "unit": "GB/s",
+                         "frac": gbs / B.peaks.get("hbm_gbs", 6650.0),
+                         "algorithmic_bytes": W.nx * W.ny * 16, "peak_source": B.peak_src}}
+    # the deflection at a short list of observed image positions against the whole catalogue (P:140, step 1)
+    cols = W.lenses.shape[1]
+    pts_fn = {5: lt.lt_gradient_points_sie, 6: lt.lt_gradient_points_nfw}.get(cols, lt.lt_gradient_points)
+    rng = np.random.default_rng(W.seed + 78)
+    Ld = r.d_lenses
+    line["points"] = {}
+    for n_pts in (128, 4096):
+        pts = torch.from_numpy(np.stack([rng.uniform(W.x_min, W.x_min + W.dx * (W.nx - 1), n_pts),
+                                         rng.uniform(W.y_min, W.y_min + W.dx * (W.ny - 1), n_pts)], axis=1)).cuda()
+        po = torch.empty((n_pts, 2), dtype=torch.float64, device="cuda")
+        wsp = lt.alloc_workspace(len(W.lenses), 1, 1, lt.LT_FP64)
+        ts = []
+        for it in range(13):
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(20):           # back to back: per-call time of a stream of calls
+                pts_fn(Ld, pts, out=po, workspace=wsp)
+            b_.record()
+            torch.cuda.synchronize()
+            if it >= 3:
+                ts.append(a.elapsed_time(b_) / 20)
+        us = sum(ts) / len(ts) * 1e3
+        line["points"]["%d_points" % n_pts] = {"us": us, "n_lenses": len(W.lenses),
+                                               "value": n_pts * len(W.lenses) / (us * 1e-6), "unit": UNIT}
+    # one whole chi^2 evaluation (P:140, eq. 11) as a user composes it from the library's calls, on one stream with no
+    # host round trip.  The "observed" catalogue is synthetic: the images the model itself predicts for 16 source points
+    # (so chi^2 must come out at the interpolation error of the triangles, ~0).
+    src16 = src_all[:16].contiguous()
+    h0, n0 = lt.lt_find_images(r.out, W.x_min, W.y_min, W.dx, 1.0, src16)
+    rec, _ = lt.hits_to_numpy(h0, n0)
+    obs_np = np.stack([rec["x"], rec["y"]], axis=1)
+    # keep the images the exact deflection lenses back onto their source (drops the spurious "central images" the
+    # triangles around a singular or unresolved lens centre produce)
+    back = obs_np - pts_fn(Ld, torch.from_numpy(obs_np).cuda()).cpu().numpy()
+    keep = np.hypot(*(back - src16.cpu().numpy()[rec["source"]]).T) < 0.05 * W.dx
+    rec, obs_np = rec[keep], obs_np[keep]
+    off_np = np.searchsorted(rec["source"], np.arange(17)).astype(np.int32)
+    d_obs, d_off = torch.from_numpy(obs_np).cuda(), torch.from_numpy(off_np).cuda()
+    d_sig = torch.full((len(obs_np),), 0.5, dtype=torch.float64, device="cuda")
+    ws_p = lt.alloc_workspace(len(W.lenses), 1, 1, lt.LT_FP64)
+    ws_mixed = lt.alloc_workspace(len(W.lenses), W.nx, W.ny, lt.LT_MIXED)
+
+    def chi2_once(map_mode, ws_map):
+        al = pts_fn(Ld, d_obs, workspace=ws_p)
+        bary = lt.lt_source_barycentres(d_obs, al, d_off, 1.0)
+        gmap = r.grid(Ld, W.x_min, W.y_min, W.dx, W.nx, W.ny, map_mode, mixed=r.mixed, out=r.out, workspace=ws_map)
+        lt.lt_find_images(gmap, W.x_min, W.y_min, W.dx, 1.0, bary, hits=hits, n_hits=n_hits)
+        return lt.lt_chi2(d_obs, d_sig, d_off, hits, n_hits)
+
+    def chi2_timed(map_mode, ws_map):
+        ts = []
+        for it in range(6):
+            flush.fill_(1)
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            res, terms = chi2_once(map_mode, ws_map)
+            b_.record()
+            torch.cuda.synchronize()
+            if it >= 2:
+                ts.append(a.elapsed_time(b_))
+        return sum(ts) / len(ts), lt.chi2_to_python(res), terms.cpu().numpy()
+    # the same evaluation on the mixed-precision map (the paper's proposal: P:330)
+    ms_mx, (c2_mx, n_m_mx, n_u_mx), terms_mx = chi2_timed(lt.LT_MIXED, ws_mixed)
+    ms_c2, (c2, n_m, n_u), terms_64 = chi2_timed(lt.LT_FP64, r.ws)
+    # sigma * sqrt(term) is the distance between an observed image and its predicted counterpart
+    shift = 0.5 * np.nanmax(np.abs(np.sqrt(terms_mx) - np.sqrt(terms_64))) if len(terms_64) else 0.0
+    line["chi2_chain"] = {"ms_per_evaluation": ms_c2, "n_systems": 16, "n_images": int(len(obs_np)),
+                          "chi2": c2, "n_matched": n_m, "n_unmatched": n_u, "sigma_arcsec": 0.5,
+                          "mixed_map": {"ms_per_evaluation": ms_mx, "chi2": c2_mx, "n_matched": n_m_mx,
+                                        "n_unmatched": n_u_mx,
+                                        "max_change_of_image_distance_arcsec": float(shift)},
+                          "calls": "lt_gradient_points -> lt_source_barycentres -> lt_gradient_grid -> "
+                                   "lt_find_images -> lt_chi2",
+                          "catalogue": "synthetic: the model's own predicted images of 16 source points that the exact "
+                                       "deflection lenses back to within 0.05 pixel of their source"}
+
+
+def run_ours(args, W):
+    B = Bench(args)
+    torch, lt, world, rank = B.torch, B.lt, B.world, B.rank
+    block = None
+    if args.shard == "rows":
+        from paper_1902_03252_b200 import shard
+        block = shard.local_block(W.y_min, W.dx, W.ny, rank, world, halo_below=(args.mode == "mixed"))
+        if block.j1 == block.j0:
+            raise RuntimeError("--shard rows: more ranks than rows")
+    elif world > 1:
+        W = make_workload(args, seed_offset=rank)                                           # own catalogue per rank
+    sampler = ClockSampler(physical_index(B.local))
+
+    # ---- headline: the requested mode, device-resident inputs; then e2e through the host-buffer entry point
+    sampler.start()
+    m = B.measure(W, args.mode, args.steps, args.warmup, block=block)
+    r = m["runner"]
+    total_units = r.units if args.shard == "rows" else world * r.units
+    value = total_units / (m["ms"] * 1e-3)
+    mh = B.measure(W, args.mode, max(3, min(args.steps, 20)), max(3, min(args.warmup, 5)), host=True, block=block)
+    ms_e2e, h2d, d2h = mh["ms"], mh["runner"].h2d, mh["runner"].d2h
+    del mh
+    clocks = sampler.stop()
+    B.sm_max = float(clocks.get("sm_max_mhz") or B.sm_max)
+    B.sm_run = float(clocks.get("sm_mhz") or B.sm_max)        # median SM clock sampled during the timed region
+
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_median": spread["median"],
-            "ms_per_step_best": spread["best"], "ms_per_step_worst": spread["worst"],
-            "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": m["ms"], "ms_per_step_median": m["spread"]["median"],
+            "ms_per_step_best": m["spread"]["best"], "ms_per_step_worst": m["spread"]["worst"],
+            "higher_is_better": True, "scaling": "strong" if args.shard == "rows" else "weak",
             "vs_baseline": (value / PAPER_V100_SIE[args.mode] if (args.model == "sie" and world == 1 and
                                                                   args.mode in PAPER_V100_SIE) else None),
             "dtype": DTYPE[args.mode], "data": "synthetic",
             "config": {"workload": W.name, "n_lens": int(len(W.lenses)), "nx": W.nx, "ny": W.ny, "seed": W.seed,
-                       "mode": args.mode, "mixed_rule": ("paper constants" if M_MAX <= 0 else "calibrated, M_max = %g" % M_MAX),
-                       "parallelism": "dp%d (independent catalogues, no exchange)" % world,
+                       "mode": args.mode,
+                       "mixed_rule": ("paper constants" if args.m_max <= 0 else "calibrated, M_max = %g" % args.m_max),
+                       "parallelism": ("rows/%d (one map, contiguous row blocks, catalogue replicated, no exchange)" % world
+                                       if args.shard == "rows" else
+                                       "dp%d (independent catalogues, no exchange)" % world),
                        "l2": "256 MiB buffer overwritten between timed steps", "inputs": "resident in HBM"},
             "clocks": clocks,
-            "e2e": {"value": world * r.units / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
-                    "h2d_bytes_per_step": r.h2d, "d2h_bytes_per_step": r.d2h,
+            "e2e": {"value": total_units / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "lt_gradient_grid_host: pinned host catalogue read over PCIe by the precompute kernel, map stored into "
                            "pinned host memory over PCIe by the gradient kernels while they compute (no staging copy)"},
             "gpu_launches": r.launches * args.steps, "gpu_launches_per_step": r.launches,
-            "roofline": roofline(args.mode, ms_kernel_main, r.units, extra.get("flagged_fraction", 1.0))}
-    line.update(extra)
+            "roofline": B.roofline(W, m, args.mode)}
+    line.update(m["extra"])
+    if args.shard == "rows":
+        # per-rank step times (a block's rows cost the same everywhere: the spread is the load imbalance of the cut)
+        t = torch.zeros(world, dtype=torch.float64, device="cuda")
+        t[rank] = m["ms_local"]
+        if B.dist is not None:
+            B.dist.all_reduce(t)
+        line["shard"] = {"rows_per_rank": [j1 - j0 for j0, j1 in shard.row_blocks(W.ny, world)],
+                         "halo_rows_rank0": block.halo, "ms_per_rank": [float(v) for v in t.cpu()]}
+        if args.gather:
+            own = r.out[block.halo:]
+            ts = []
+            for it in range(8):
+                torch.cuda.synchronize()
+                B.barrier()
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                full = shard.all_gather_rows(own, W.ny, W.nx, rank, world) if B.dist is not None else own
+                b_.record()
+                torch.cuda.synchronize()
+                if it >= 3:
+                    ts.append(a.elapsed_time(b_))
+                del full
+            line["shard"]["all_gather_ms"] = B.max_over_ranks(sum(ts) / len(ts))
 
     if not args.no_extras:
-        modes = {args.mode: {"value": value, "ms_per_step": ms, **extra}}
-        for m in MODES:
-            if m == args.mode:
+        # ---- the other modes on the same workload
+        sampled, flags_s = {}, None
+        got, f = B.sample_map(W, r) if block is None else (None, None)
+        if got is not None:
+            sampled[args.mode] = got
+            flags_s = f
+        modes = {args.mode: {"value": value, "ms_per_step": m["ms"], "kernel_ms": m["ms_kernel"],
+                             "roofline_frac_nominal": line["roofline"]["frac"], **m["extra"]}}
+        mixed_params = r.mixed_params
+        for mode in MODES:
+            if mode == args.mode:
                 continue
-            rm, ms_m, ex = measure(m, max(3, min(args.steps, 50)), max(3, min(args.warmup, 5)))
-            modes[m] = {"value": world * rm.units / (ms_m * 1e-3), "ms_per_step": ms_m, **ex,
-                        "kernel_ms": rm.ms_kernel,
-                        "roofline_frac_nominal": roofline(m, rm.ms_kernel, rm.units,
-                                                          ex.get("flagged_fraction", 1.0))["frac"]}
+            mm = B.measure(W, mode, max(3, min(args.steps, 10)), max(3, min(args.warmup, 5)), block=block)
+            rm = mm["runner"]
+            tu = rm.units if args.shard == "rows" else world * rm.units
+            modes[mode] = {"value": tu / (mm["ms"] * 1e-3), "ms_per_step": mm["ms"], "kernel_ms": mm["ms_kernel"],
+                           "roofline_frac_nominal": B.roofline(W, mm, mode)["frac"], **mm["extra"]}
+            ex = B.executed(rm.model, mode, mm["ms_kernel"], rm.units_local * mm["extra"].get("flagged_fraction", 1.0))
+            if ex:
+                modes[mode]["frac_of_floor"] = ex["frac_of_floor"]
+            if block is None:
+                got, f = B.sample_map(W, rm)
+                sampled[mode] = got
+                flags_s = f if f is not None else flags_s
+            del mm, rm
+        if "mixed" in modes and "fp64" in modes:
+            # the paper's Table 2 comparison on THIS workload: < 1 only where the rule flags a minority of the pixels
+            modes["mixed"]["time_vs_fp64"] = modes["mixed"]["ms_per_step"] / modes["fp64"]["ms_per_step"]
         line["modes"] = modes
-        if rank == 0:
+
+        if rank == 0 and world == 1:
             # the same step replayed from a CUDA graph (what an MCMC loop would do): launch gaps removed
             gs = torch.cuda.Stream()
             graph = torch.cuda.CUDAGraph()
@@ -442,8 +734,8 @@ def run_ours(args, W):
                     r.grid(r.d_lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, r.code, mixed=r.mixed, out=r.out,
                            workspace=r.ws, stream=gs)
             ts = []
-            for it in range(13):
-                flush.fill_(1)
+            for it in range(8):
+                B.flush.fill_(1)
                 a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 a.record()
                 graph.replay()
@@ -452,133 +744,46 @@ def run_ours(args, W):
                 if it >= 3:
                     ts.append(a.elapsed_time(b_))
             line["cuda_graph_replay"] = {"ms_per_step": sum(ts) / len(ts), "value": r.units / (sum(ts) / len(ts) * 1e-3)}
-        if rank == 0 and args.mode == "fp64":
-            # the consumer of the map (section 2.2.2): triangle search for 64 synthetic source points on the
-            # fp64 map just computed; memory-bound when the sources are few: 16 B per node read once
-            import numpy as np
-            rng = np.random.default_rng(W.seed + 77)
-            src_all = torch.from_numpy(rng.normal(0.0, 8.0, (64, 2)) + W.lenses[0, :2]).cuda()
-            hits = torch.empty((1 << 16, 32), dtype=torch.uint8, device="cuda")
-            n_hits = torch.empty(1, dtype=torch.int32, device="cuda")
-            line["find_images"] = {}
-            for n_src in (4, 64):                 # few sources: bound by reading the map; many: by the source loop
-                src = src_all[:n_src].contiguous()
-                ts = []
-                for it in range(8):
-                    flush.fill_(1)
-                    a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record()
-                    lt.lt_find_images(r.out, W.x_min, W.y_min, W.dx, 1.0, src, hits=hits, n_hits=n_hits)
-                    b_.record()
-                    torch.cuda.synchronize()
-                    if it >= 3:
-                        ts.append(a.elapsed_time(b_))
-                ms_fi = sum(ts) / len(ts)
-                gbs = W.nx * W.ny * 16 / (ms_fi * 1e-3) / 1e9
-                line["find_images"]["%d_sources" % n_src] = {
-                    "ms": ms_fi, "images_found": int(n_hits.item()),
-                    "cells_per_s": (W.nx - 1) * (W.ny - 1) / (ms_fi * 1e-3),
-                    "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
-                                 "frac": gbs / peaks.get("hbm_gbs", 6650.0),
-                                 "algorithmic_bytes": W.nx * W.ny * 16, "peak_source": peak_src}}
-        if rank == 0 and args.mode == "fp64":
-            # the other call of the chi^2 algorithm (step 1): the deflection at a short list of observed image
-            # positions against the whole catalogue -- one warp per point, precompute kernel included
-            import numpy as np
-            pts_fn = {5: lt.lt_gradient_points_sie, 6: lt.lt_gradient_points_nfw}.get(W.lenses.shape[1], lt.lt_gradient_points)
-            rng = np.random.default_rng(W.seed + 78)
-            Ld = torch.from_numpy(W.lenses).cuda()
-            line["points"] = {}
-            for n_pts in (128, 4096):
-                pts = torch.from_numpy(np.stack([rng.uniform(W.x_min, W.x_min + W.dx * (W.nx - 1), n_pts),
-                                                 rng.uniform(W.y_min, W.y_min + W.dx * (W.ny - 1), n_pts)], axis=1)).cuda()
-                po = torch.empty((n_pts, 2), dtype=torch.float64, device="cuda")
-                wsp = lt.alloc_workspace(len(W.lenses), 1, 1, lt.LT_FP64)
-                ts = []
-                for it in range(13):
-                    a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record()
-                    for _ in range(20):           # back to back: per-call time of a stream of calls
-                        pts_fn(Ld, pts, out=po, workspace=wsp)
-                    b_.record()
-                    torch.cuda.synchronize()
-                    if it >= 3:
-                        ts.append(a.elapsed_time(b_) / 20)
-                us = sum(ts) / len(ts) * 1e3
-                line["points"]["%d_points" % n_pts] = {"us": us, "n_lenses": len(W.lenses),
-                                                       "value": n_pts * len(W.lenses) / (us * 1e-6), "unit": UNIT}
-        if rank == 0 and args.mode == "fp64":
-            # one whole chi^2 evaluation (eq. 11) as a user composes it from the library's calls, on one stream
-            # with no host round trip.  The "observed" catalogue is synthetic: the images the model itself predicts for 16
-            # source points (so chi^2 must come out at the interpolation error of the triangles, ~0).
-            src16 = src_all[:16].contiguous()
-            h0, n0 = lt.lt_find_images(r.out, W.x_min, W.y_min, W.dx, 1.0, src16)
-            rec, _ = lt.hits_to_numpy(h0, n0)
-            obs_np = np.stack([rec["x"], rec["y"]], axis=1)
-            # keep the images the exact deflection lenses back onto their source (drops the spurious "central images" the
-            # triangles around a singular or unresolved lens centre produce)
-            back = obs_np - pts_fn(Ld, torch.from_numpy(obs_np).cuda()).cpu().numpy()
-            keep = np.hypot(*(back - src16.cpu().numpy()[rec["source"]]).T) < 0.05 * W.dx
-            rec, obs_np = rec[keep], obs_np[keep]
-            off_np = np.searchsorted(rec["source"], np.arange(17)).astype(np.int32)
-            d_obs, d_off = torch.from_numpy(obs_np).cuda(), torch.from_numpy(off_np).cuda()
-            d_sig = torch.full((len(obs_np),), 0.5, dtype=torch.float64, device="cuda")
-            grid_fn = r.grid
-            ws_p = lt.alloc_workspace(len(W.lenses), 1, 1, lt.LT_FP64)
-
-            ws_mixed = lt.alloc_workspace(len(W.lenses), W.nx, W.ny, lt.LT_MIXED)
-
-            def chi2_once(map_mode, ws_map):
-                al = pts_fn(Ld, d_obs, workspace=ws_p)
-                bary = lt.lt_source_barycentres(d_obs, al, d_off, 1.0)
-                gmap = grid_fn(Ld, W.x_min, W.y_min, W.dx, W.nx, W.ny, map_mode, out=r.out, workspace=ws_map)
-                lt.lt_find_images(gmap, W.x_min, W.y_min, W.dx, 1.0, bary, hits=hits, n_hits=n_hits)
-                return lt.lt_chi2(d_obs, d_sig, d_off, hits, n_hits)
-
-            def chi2_timed(map_mode, ws_map):
-                ts = []
-                for it in range(8):
-                    flush.fill_(1)
-                    a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record()
-                    res, terms = chi2_once(map_mode, ws_map)
-                    b_.record()
-                    torch.cuda.synchronize()
-                    if it >= 3:
-                        ts.append(a.elapsed_time(b_))
-                return sum(ts) / len(ts), lt.chi2_to_python(res), terms.cpu().numpy()
-            # the same evaluation on the mixed-precision map (the paper's proposal: P:330), paper constants
-            ms_mx, (c2_mx, n_m_mx, n_u_mx), terms_mx = chi2_timed(lt.LT_MIXED, ws_mixed)
-            ms_c2, (c2, n_m, n_u), terms_64 = chi2_timed(lt.LT_FP64, r.ws)
-            # sigma * sqrt(term) is the distance between an observed image and its predicted counterpart
-            shift = 0.5 * np.nanmax(np.abs(np.sqrt(terms_mx) - np.sqrt(terms_64))) if len(terms_64) else 0.0
-            line["chi2_chain"] = {"ms_per_evaluation": ms_c2, "n_systems": 16, "n_images": int(len(obs_np)),
-                                  "chi2": c2, "n_matched": n_m, "n_unmatched": n_u, "sigma_arcsec": 0.5,
-                                  "mixed_map": {"ms_per_evaluation": ms_mx, "chi2": c2_mx, "n_matched": n_m_mx,
-                                                "n_unmatched": n_u_mx,
-                                                "max_change_of_image_distance_arcsec": float(shift)},
-                                  "calls": "lt_gradient_points -> lt_source_barycentres -> lt_gradient_grid -> "
-                                           "lt_find_images -> lt_chi2",
-                                  "catalogue": "synthetic: the model's own predicted images of 16 source points that the exact "
-                                               "deflection lenses back to within 0.05 pixel of their source"}
-        if rank == 0:
+            del graph
+            if args.mode == "fp64":
+                consumers(B, W, r, line)
             p64, p32 = lt.lt_peak_probe(0, 1 << 15), lt.lt_peak_probe(1, 1 << 16)
             line["peak_probe"] = {"fp64_tflops": p64 / 1e12, "fp32_tflops": p32 / 1e12,
                                   "how": "dependent-free FMA chains, full grid, same process"}
             line["roofline"]["frac_of_probe"] = line["roofline"]["achieved"] / (
                 (p64 if LANES[args.mode] == 64 else p32) / 1e12)
+
+        # ---- the other BASELINE configs and the paper's own benchmark, three modes each
+        cfg_samples = {}
+        if rank == 0 and world == 1 and not args.no_configs and args.model == "dpie" and not args.paper_regime:
+            from paper_1902_03252_b200 import workloads
+            del m, r
+            torch.cuda.empty_cache()
+            line["configs"] = {}
+            others = [workloads.make(c) for c in (1, 2, 4) if c != args.config] + [workloads.make_sie("paper")]
+            for Wc in others:
+                entry, smp, fl, mp = B.three_modes(Wc, 5, 3)
+                line["configs"][Wc.name] = entry
+                cfg_samples[Wc.name] = (Wc, smp, fl, mp)
+                torch.cuda.empty_cache()
+
         if rank == 0 and world == 1:
-            # the cpu_baseline leg: with run_reference the one place bench.py runs the oracle (inside time_oracle)
+            # ---- the cpu_baseline leg: the one place (with run_reference) where bench.py runs the oracle -- it times the
+            # `double` instantiation on a row sample and evaluates the long-double oracle at the parity sample
             stride, rows = oracle_sample(W, args.cpu_seconds)
             v, dt = time_oracle(W, stride)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
                                     "seconds": dt,
                                     "sample": "rows 0,%d,... (%d of %d rows) of %s, `double` instantiation, "
                                               "OpenMP over rows" % (stride, rows, W.ny, W.name)}
+            if sampled:
+                line["parity"] = oracle_parity(W, sampled, flags_s, mixed_params)
+            for name, (Wc, smp, fl, mp) in cfg_samples.items():
+                line["configs"][name]["parity"] = oracle_parity(Wc, smp, fl, mp)
     if rank == 0:
         print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    if B.dist is not None:
+        B.dist.destroy_process_group()
 
 
 def make_workload(args, seed_offset=0):
@@ -590,16 +795,10 @@ def make_workload(args, seed_offset=0):
     return workloads.make(args.config, paper_regime=args.paper_regime, seed_offset=seed_offset)
 
 
-M_MAX = 0.0
-
-
 def main():
-    global M_MAX
     args = parse_args()
-    M_MAX = args.m_max
     if args.warmup < 3:
         args.warmup = 3
-    from paper_1902_03252_b200 import workloads
     W = make_workload(args)
     if args.impl == "reference":
         run_reference(args, W)

@@ -270,6 +270,8 @@ int lt_chi2(const double* d_theta_obs, const double* d_sigma, const int* d_offse
  * programmatic-dependent-launch attribute.  Results do not depend on
  * any of them except that the fp32 tile centre moves with the pixels per thread of the launch
  * that owns the pixel.  Returns LT_ERR_BAD_SIZE on a negative value.
+ * Thread safety: the knobs are independent atomics; a launch racing this call sees each knob either old or new.  They
+ * are measurement and test hooks, not per-call state: set them before the threads that launch are started.
  */
 int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_sm, int single_launch);
 
@@ -298,6 +300,12 @@ int lt_mixed_last_stats(const void* d_workspace, void* cuda_stream, lt_mixed_sta
  * kept in the workspace into d_flags_out (device).  Asynchronous on cuda_stream. */
 int lt_mixed_last_flags(const void* d_workspace, int n_lens, int nx, int ny, unsigned char* d_flags_out,
                         void* cuda_stream);
+
+/* After an LT_MIXED call: copies the single precision map of its first step ("first, we compute the gradient in SP
+ * for every pixel"; nx*ny*2 floats, layout of the output) kept in the workspace into d_sp_out (device).  This is the map
+ * eq. 24-28 were evaluated on, so the flag map of lt_mixed_last_flags is a function of it and of the lens
+ * centres alone.  Asynchronous on cuda_stream. */
+int lt_mixed_last_sp_map(const void* d_workspace, int n_lens, int nx, int ny, float* d_sp_out, void* cuda_stream);
 
 /* FMA-chain microbenchmarks used by bench.py to confirm the FP64 / FP32 peaks on the device in the same run
  * (SURVEY 8(d)): runs `iters` dependent-free FMAs per thread on a full grid; returns achieved FLOP/s in *flops_out

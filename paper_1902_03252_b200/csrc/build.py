@@ -14,8 +14,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 PKG = os.path.dirname(HERE)
 LIB = os.path.join(PKG, "liblt_gradient.so")
 SOURCES = ["lt_api.cu"]
-DEPS = ["lt_api.cu", "lt_kernels.cuh", "lt_mixed.cuh", "lt_math.cuh", "lt_pack.cuh", "lt_images.cuh",
-        os.path.join("..", "..", "include", "lt_gradient.h")]
+
+
+def deps():
+    """Every source the library is built from: all *.cu / *.cuh of this folder and the C-ABI header."""
+    here = sorted(f for f in os.listdir(HERE) if f.endswith((".cu", ".cuh")))
+    return here + [os.path.join("..", "..", "include", "lt_gradient.h"), "build.py"]
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--fmad=false",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -31,7 +36,7 @@ def up_to_date():
     if not os.path.exists(LIB):
         return False
     t = os.path.getmtime(LIB)
-    return all(os.path.getmtime(os.path.join(HERE, d)) <= t for d in DEPS + ["build.py"])
+    return all(os.path.getmtime(os.path.join(HERE, d)) <= t for d in deps())
 
 
 def build(force=False, verbose=False):

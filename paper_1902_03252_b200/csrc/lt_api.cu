@@ -5,7 +5,11 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <atomic>
+#include <map>
 #include <mutex>
+#include <tuple>
+#include <utility>
 
 #include "../../include/lt_gradient.h"
 #include "lt_mixed.cuh"
@@ -26,8 +30,11 @@ namespace {
 
 thread_local int g_last_cuda_error = 0;
 
+// lt_set_tuning's knobs: process-wide, each one an atomic int read with relaxed loads on the launch path, so a call
+// that races lt_set_tuning sees every knob either old or new (the knobs are independent of one another)
 struct Tuning {
-  int ppt64 = 0, ppt32 = 0, chunk64 = 0, chunk32 = 0, ctas_per_sm = 0, single_launch = 0, staged_host_output = 0, points_per_thread = 0, no_dependent_launch = 0;
+  std::atomic<int> ppt64{0}, ppt32{0}, chunk64{0}, chunk32{0}, ctas_per_sm{0}, single_launch{0}, staged_host_output{0},
+      points_per_thread{0}, no_dependent_launch{0};
 };
 Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
@@ -95,40 +102,66 @@ int device_info(DeviceInfo& d) {
   return LT_OK;
 }
 
-// resident CTAs of `kernel` on the whole device with `smem` bytes of dynamic shared memory (opt-in set); cached per
-// (kernel, smem) because the two runtime queries cost microseconds on a path that launches sub-millisecond kernels
+// Per-kernel facts, cached for the life of the process in maps that never evict (one entry per kernel instantiation and
+// device; one per (kernel, device, dynamic shared memory) for the occupancy): the runtime queries cost microseconds on a
+// path that launches sub-millisecond kernels.  The first use of a kernel opts it in ONCE to the largest dynamic shared
+// memory it can ever be given (the device's opt-in limit minus the kernel's own static shared memory), so the attribute
+// is never lowered and a launch from another host thread with a larger chunk cannot fail on it.
+struct KernelInfo {
+  size_t static_smem = 0, max_dynamic = 0;
+};
+std::mutex g_kernel_mu;
 template <class K>
-int resident_ctas(K kernel, size_t smem, const DeviceInfo& d, long long& resident) {
-  struct Entry { const void* fn; size_t smem; int device, occ; };
-  static Entry cache[32];                  // process-wide (the opt-in is a property of the function, not the thread)
-  static int n_cache = 0;
-  static std::mutex mu;
-  std::lock_guard<std::mutex> lock(mu);
-  const void* key = reinterpret_cast<const void*>(kernel);
-  int occ = 0;
-  for (int i = 0; i < n_cache; ++i)
-    if (cache[i].fn == key && cache[i].smem == smem && cache[i].device == d.device) occ = cache[i].occ;
-  if (occ == 0) {
-    if (n_cache == 32) n_cache = 0;        // full: start over (every kernel then re-opts in on its next miss)
-    size_t opted = 0;                      // within the cache's lifetime the opt-in only grows
-    for (int i = 0; i < n_cache; ++i)
-      if (cache[i].fn == key && cache[i].device == d.device && cache[i].smem > opted) opted = cache[i].smem;
-    if (smem > opted)
-      LT_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, LT_THREADS, smem));
-    if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources);
-    cache[n_cache++] = Entry{key, smem, d.device, occ};
+int kernel_info(K kernel, const DeviceInfo& d, KernelInfo& out) {
+  static std::map<std::pair<const void*, int>, KernelInfo> cache;
+  const std::pair<const void*, int> key(reinterpret_cast<const void*>(kernel), d.device);
+  std::lock_guard<std::mutex> lock(g_kernel_mu);
+  auto it = cache.find(key);
+  if (it == cache.end()) {
+    cudaFuncAttributes fa;
+    LT_CUDA(cudaFuncGetAttributes(&fa, kernel));
+    KernelInfo ki;
+    ki.static_smem = fa.sharedSizeBytes;
+    ki.max_dynamic = d.smem_optin > ki.static_smem ? d.smem_optin - ki.static_smem : 0;
+    LT_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ki.max_dynamic));
+    it = cache.emplace(key, ki).first;
   }
-  if (g_tuning.ctas_per_sm > 0 && g_tuning.ctas_per_sm < occ) occ = g_tuning.ctas_per_sm;
+  out = it->second;
+  return LT_OK;
+}
+
+// resident CTAs of `kernel` (CTAs of `threads` threads) on the whole device with `smem` bytes of dynamic shared memory
+template <class K>
+int resident_ctas(K kernel, size_t smem, const DeviceInfo& d, long long& resident, int threads = LT_THREADS) {
+  KernelInfo ki;
+  const int rc = kernel_info(kernel, d, ki);
+  if (rc != LT_OK) return rc;
+  if (smem > ki.max_dynamic) return cuda_fail(cudaErrorLaunchOutOfResources);
+  static std::map<std::tuple<const void*, int, size_t>, int> cache;
+  const std::tuple<const void*, int, size_t> key(reinterpret_cast<const void*>(kernel), d.device, smem);
+  int occ = 0;
+  {
+    std::lock_guard<std::mutex> lock(g_kernel_mu);
+    auto it = cache.find(key);
+    if (it != cache.end()) occ = it->second;
+  }
+  if (occ == 0) {
+    LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem));
+    if (occ < 1) return cuda_fail(cudaErrorLaunchOutOfResources);
+    std::lock_guard<std::mutex> lock(g_kernel_mu);
+    cache[key] = occ;
+  }
+  const int cap = g_tuning.ctas_per_sm;
+  if (cap > 0 && cap < occ) occ = cap;
   resident = (long long)occ * d.sms;
   return LT_OK;
 }
 
 // persistent grid: min(#work groups, resident CTAs)
 template <class K>
-int grid_for(K kernel, size_t smem, long long n_work, const DeviceInfo& d, int& grid) {
+int grid_for(K kernel, size_t smem, long long n_work, const DeviceInfo& d, int& grid, int threads = LT_THREADS) {
   long long g = 0;
-  const int rc = resident_ctas(kernel, smem, d, g);
+  const int rc = resident_ctas(kernel, smem, d, g, threads);
   if (rc != LT_OK) return rc;
   if (g > n_work) g = n_work;
   if (g < 1) g = 1;
@@ -136,13 +169,19 @@ int grid_for(K kernel, size_t smem, long long n_work, const DeviceInfo& d, int& 
   return LT_OK;
 }
 
-int pick_chunk(int n_lens, int wanted, size_t rec_bytes, const DeviceInfo& d) {
-  int chunk = wanted;
-  const int max_chunk = (int)((d.smem_optin - 4096) / rec_bytes   /* static smem: the range-reduction tables */);
+// lenses per shared-memory chunk: the wanted number, clamped to the catalogue and to what fits beside the kernel's own
+// static shared memory (the range-reduction tables) under the device's opt-in limit
+template <class K>
+int pick_chunk(K kernel, int n_lens, int wanted, size_t rec_bytes, const DeviceInfo& d, int& chunk) {
+  KernelInfo ki;
+  const int rc = kernel_info(kernel, d, ki);
+  if (rc != LT_OK) return rc;
+  chunk = wanted;
+  const int max_chunk = (int)(ki.max_dynamic / rec_bytes);
   if (chunk > max_chunk) chunk = max_chunk;
   if (chunk > n_lens) chunk = n_lens;
   if (chunk < 1) chunk = 1;
-  return chunk;
+  return LT_OK;
 }
 
 // pixels per thread: the largest of the candidates that still gives every SM about two tiles
@@ -227,12 +266,14 @@ int launch_waves(int ppt, const GridArgs& a, Fn fn) {
 template <class M, int PPT, int MINB>
 int launch_f64_ppt(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
                    const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end, long long* resident) {
-  const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
-                               sizeof(typename Rec64<M>::type), d);
+  int chunk = 1, grid = 1;
+  const int wanted = g_tuning.chunk64;
+  int rc = pick_chunk(lt_grad_f64_kernel<M, PPT, MINB>, a.n_lens, wanted > 0 ? wanted : kDefaultChunk64,
+                      sizeof(typename Rec64<M>::type), d, chunk);
+  if (rc != LT_OK) return rc;
   const size_t smem = (size_t)chunk * sizeof(typename Rec64<M>::type);
   if (resident) return resident_ctas(lt_grad_f64_kernel<M, PPT, MINB>, smem, d, *resident);
-  int grid = 1;
-  const int rc = grid_for(lt_grad_f64_kernel<M, PPT, MINB>, smem, end - begin, d, grid);
+  rc = grid_for(lt_grad_f64_kernel<M, PPT, MINB>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
   LT_CUDA(launch_dependent(lt_grad_f64_kernel<M, PPT, MINB>, grid, LT_THREADS, smem, st, l64, t64, a.n_lens, chunk, a.x_min,
                            a.y_min, a.dx, a.nx, a.ny, tiles_x, (int)begin, (int)end, out));
@@ -259,12 +300,14 @@ template <class M, int PPT, int MINB, bool WIDE>
 int launch_f32_ppt(const typename Rec64<M>::type* l64, const typename Rec32<M>::type* l32, const LtTables<float>* t32,
                    const GridArgs& a, float2* out, double2* out_wide, const DeviceInfo& d, cudaStream_t st,
                    int tiles_x, long long begin, long long end, long long* resident) {
-  const int chunk = pick_chunk(a.n_lens, g_tuning.chunk32 > 0 ? g_tuning.chunk32 : kDefaultChunk32,
-                               sizeof(typename Rec32<M>::type), d);
+  int chunk = 1, grid = 1;
+  const int wanted = g_tuning.chunk32;
+  int rc = pick_chunk(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, a.n_lens, wanted > 0 ? wanted : kDefaultChunk32,
+                      sizeof(typename Rec32<M>::type), d, chunk);
+  if (rc != LT_OK) return rc;
   const size_t smem = (size_t)chunk * sizeof(typename Rec32<M>::type);
   if (resident) return resident_ctas(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, smem, d, *resident);
-  int grid = 1;
-  const int rc = grid_for(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, smem, end - begin, d, grid);
+  rc = grid_for(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, smem, end - begin, d, grid);
   if (rc != LT_OK) return rc;
   LT_CUDA(launch_dependent(lt_grad_f32_kernel<M, PPT, MINB, WIDE>, grid, LT_THREADS, smem, st, l64, l32, t32, a.n_lens, chunk,
                            a.x_min, a.y_min, a.dx, a.nx, a.ny, tiles_x, (int)begin, (int)end, out, out_wide));
@@ -299,11 +342,13 @@ template <class M, bool FROM_LIST>
 int launch_list(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, const unsigned int* list, const LtWsHeader* hdr,
                 const double2* points, long long n_points, long long max_work, double2* out, const DeviceInfo& d,
                 cudaStream_t st) {
-  const int chunk = pick_chunk(a.n_lens, g_tuning.chunk64 > 0 ? g_tuning.chunk64 : kDefaultChunk64,
-                               sizeof(typename Rec64<M>::type), d);
+  int chunk = 1, grid = 1;
+  const int wanted = g_tuning.chunk64;
+  int rc = pick_chunk(lt_grad_list_f64_kernel<M, FROM_LIST>, a.n_lens, wanted > 0 ? wanted : kDefaultChunk64,
+                      sizeof(typename Rec64<M>::type), d, chunk);
+  if (rc != LT_OK) return rc;
   const size_t smem = (size_t)chunk * sizeof(typename Rec64<M>::type);
-  int grid = 1;
-  const int rc = grid_for(lt_grad_list_f64_kernel<M, FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
+  rc = grid_for(lt_grad_list_f64_kernel<M, FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
   if (rc != LT_OK) return rc;
   KernelEvents ke(st, FROM_LIST);
   LT_CUDA(launch_dependent(lt_grad_list_f64_kernel<M, FROM_LIST>, grid, LT_THREADS, smem, st, l64, t64, a.n_lens, chunk,
@@ -454,7 +499,7 @@ int gradient_points_impl(const void* d_lenses, int n_lens, const double* d_point
   if (n_points <= kSplitMaxPoints && !g_tuning.points_per_thread) {   /* short list: one warp per point */
     int grid = 1;
     constexpr int per_cta = LT_SPLIT_THREADS / 32;
-    rc = grid_for(lt_grad_points_split_kernel<M>, 0, (n_points + per_cta - 1) / per_cta, dev, grid);
+    rc = grid_for(lt_grad_points_split_kernel<M>, 0, (n_points + per_cta - 1) / per_cta, dev, grid, LT_SPLIT_THREADS);
     if (rc != LT_OK) return rc;
     LT_CUDA(launch_dependent(lt_grad_points_split_kernel<M>, grid, LT_SPLIT_THREADS, 0, st,
                              reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
@@ -802,6 +847,15 @@ int lt_mixed_last_flags(const void* d_workspace, int n_lens, int nx, int ny, uns
   if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
   const Layout L = make_layout(n_lens, (long long)nx * ny, true);
   LT_CUDA(cudaMemcpyAsync(d_flags_out, (const unsigned char*)d_workspace + L.flags, (size_t)nx * ny,
+                          cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+  return LT_OK;
+}
+
+int lt_mixed_last_sp_map(const void* d_workspace, int n_lens, int nx, int ny, float* d_sp_out, void* cuda_stream) {
+  if (!d_workspace || !d_sp_out) return LT_ERR_NULL_POINTER;
+  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
+  const Layout L = make_layout(n_lens, (long long)nx * ny, true);
+  LT_CUDA(cudaMemcpyAsync(d_sp_out, (const unsigned char*)d_workspace + L.sp, (size_t)nx * ny * sizeof(float2),
                           cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
   return LT_OK;
 }

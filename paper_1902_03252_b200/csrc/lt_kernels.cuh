@@ -138,10 +138,9 @@ lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ le
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
         const Rec L = sl[k];
-        const double d2 = t2 - L.y0;                                // Alg. 1 l.4
-        const auto row = M::template row<double>(d2, L);            // what the pixels of the row share
+        const auto row = M::template row_abs<double>(t2, L);        // Alg. 1 l.4 and what the pixels of the row share
 #pragma unroll
-        for (int p = 0; p < PPT; ++p) M::template interact_sky<double, true>(t1[p] - L.x0, row, L, tab, G1[p], G2[p]);  // l.3, l.5-14
+        for (int p = 0; p < PPT; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);  // l.3, l.5-14
       }
     }
     if (j < ny) {
@@ -202,13 +201,18 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
       for (int k = threadIdx.x; k < cnt; k += LT_THREADS) {
         Rec F = lens32[base + k];
         const Rec64& D = lens64[base + k];
-        const double d1 = cx - D.x0, d2 = cy - D.y0;
         if constexpr (M::kSkyFrame32) {             // sky-frame offset of the tile centre from the lens centre
-          F.x0 = (float)d1;
-          F.y0 = (float)d2;
+          F.x0 = (float)(cx - D.x0);
+          F.y0 = (float)(cy - D.y0);
         } else {                                    // (scaled) lens-frame position of the tile centre
+#ifdef LT_V_X0
+          F.x0 = (float)fma(cx, D.cx, fma(cy, D.sx, -D.x0));
+          F.y0 = (float)fma(-cx, D.sy, fma(cy, D.cy, -D.y0));
+#else
+          const double d1 = cx - D.x0, d2 = cy - D.y0;
           F.x0 = (float)fma(d1, D.cx, d2 * D.sx);
           F.y0 = (float)fma(-d1, D.sy, d2 * D.cy);
+#endif
         }
         sl[k] = F;
       }
@@ -298,10 +302,8 @@ __device__ __forceinline__ void lt_list_group(const typename M::template Rec<dou
     for (int k = 0; k < cnt; ++k) {
       const typename M::template Rec<double>::type L = sl[k];
 #pragma unroll
-      for (int p = 0; p < PPT; ++p) {
-        const double d2 = t2[p] - L.y0;
-        M::template interact_sky<double>(t1[p] - L.x0, M::template row<double>(d2, L), L, tab, G1[p], G2[p]);
-      }
+      for (int p = 0; p < PPT; ++p)
+        M::template interact_abs<double>(t1[p], M::template row_abs<double>(t2[p], L), L, tab, G1[p], G2[p]);
     }
   }
 #pragma unroll
@@ -373,12 +375,12 @@ lt_grad_points_split_kernel(const typename M::template Rec<double>::type* __rest
 #pragma unroll 1
     for (; k + 32 < n_lens; k += 64) {
       const Rec La = lens[k], Lb = lens[k + 32];
-      M::template interact_sky<double>(pt.x - La.x0, M::template row<double>(pt.y - La.y0, La), La, tab, A1, A2);
-      M::template interact_sky<double>(pt.x - Lb.x0, M::template row<double>(pt.y - Lb.y0, Lb), Lb, tab, B1, B2);
+      M::template interact_abs<double>(pt.x, M::template row_abs<double>(pt.y, La), La, tab, A1, A2);
+      M::template interact_abs<double>(pt.x, M::template row_abs<double>(pt.y, Lb), Lb, tab, B1, B2);
     }
     if (k < n_lens) {
       const Rec La = lens[k];
-      M::template interact_sky<double>(pt.x - La.x0, M::template row<double>(pt.y - La.y0, La), La, tab, A1, A2);
+      M::template interact_abs<double>(pt.x, M::template row_abs<double>(pt.y, La), La, tab, A1, A2);
     }
     double G1 = __dadd_rn(A1, B1), G2 = __dadd_rn(A2, B2);
 #pragma unroll

@@ -29,12 +29,18 @@ LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
   f = f < LT_F_MIN ? LT_F_MIN : f;           // e = 0 stays a regular point (header of lt_math.cuh)
   const double sc = r.rcore * ope, st = r.rcut * ope;
   const double rf = 1.0 / f, qf = q * rf;
-  L.x0 = r.x;
-  L.y0 = r.y;
   L.cx = qf * c;
   L.sx = qf * s;
   L.cy = rf * c;
   L.sy = rf * s;
+#ifdef LT_V_X0
+  // scaled lens-frame coordinates of the sky origin, negated: X = cx t1 + sx t2 - X0, Y = cy t2 - sy t1 - Y0
+  L.x0 = fma(L.cx, r.x, L.sx * r.y);
+  L.y0 = fma(L.cy, r.y, -(L.sy * r.x));
+#else
+  L.x0 = r.x;
+  L.y0 = r.y;
+#endif
   L.Kc = (ome * r.rcore * rf) * (ome * r.rcore * rf);  // q^2 s_c^2 / f^2
   L.Kt = (ome * r.rcut * rf) * (ome * r.rcut * rf);
   L.sc = sc * rf;
@@ -173,6 +179,22 @@ struct LtDpieModel {
     const T Y = lt_fma(-d1, L.sy, r.d2cy);           // Alg. 1 l.6, times 1/f
     interact_lens<T, GRID>(X, Y, L, tab, G1, G2);
   }
+  // the same from the absolute sky coordinates (t1, t2) of the pixel: what the fp64 kernels call
+#ifdef LT_V_X0
+  template <class T> static LT_HD Row<T> row_abs(const T t2, const LtLens<T>& L) {
+    return Row<T>{lt_fma(t2, L.sx, -L.x0), lt_fma(t2, L.cy, -L.y0)};
+  }
+  template <class T, bool GRID = false>
+  static LT_HD void interact_abs(const T t1, const Row<T>& r, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
+    interact_sky<T, GRID>(t1, r, L, tab, G1, G2);
+  }
+#else
+  template <class T> static LT_HD Row<T> row_abs(const T t2, const LtLens<T>& L) { return row<T>(t2 - L.y0, L); }
+  template <class T, bool GRID = false>
+  static LT_HD void interact_abs(const T t1, const Row<T>& r, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
+    interact_sky<T, GRID>(t1 - L.x0, r, L, tab, G1, G2);
+  }
+#endif
 };
 struct LtSieModel {
   typedef LtRawSie Raw;
@@ -191,6 +213,12 @@ struct LtSieModel {
   static LT_HD void interact_sky(const T d1, const LtSieRow<T>& r, const LtSieLens<T>& L, const LtTables<T>&, T& G1,
                                  T& G2) {
     lt_sie_interact<T>(d1, r, L, G1, G2);
+  }
+  template <class T> static LT_HD LtSieRow<T> row_abs(const T t2, const LtSieLens<T>& L) { return row<T>(t2 - L.y0, L); }
+  template <class T, bool GRID = false>
+  static LT_HD void interact_abs(const T t1, const LtSieRow<T>& r, const LtSieLens<T>& L, const LtTables<T>& tab, T& G1,
+                                 T& G2) {
+    interact_sky<T, GRID>(t1 - L.x0, r, L, tab, G1, G2);
   }
 };
 struct LtNfwModel {
@@ -212,5 +240,11 @@ struct LtNfwModel {
   static LT_HD void interact_sky(const T d1, const LtSieRow<T>& r, const LtNfwLens<T>& L, const LtTables<T>& tab, T& G1,
                                  T& G2) {
     lt_nfw_interact<T>(d1, r, L, tab, G1, G2);
+  }
+  template <class T> static LT_HD LtSieRow<T> row_abs(const T t2, const LtNfwLens<T>& L) { return row<T>(t2 - L.y0, L); }
+  template <class T, bool GRID = false>
+  static LT_HD void interact_abs(const T t1, const LtSieRow<T>& r, const LtNfwLens<T>& L, const LtTables<T>& tab, T& G1,
+                                 T& G2) {
+    interact_sky<T, GRID>(t1 - L.x0, r, L, tab, G1, G2);
   }
 };

@@ -24,7 +24,7 @@ SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defa
            "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images", "lt_mixed_rule",
            "lt_source_barycentres", "lt_chi2",
            "lt_gradient_grid_nfw", "lt_gradient_points_nfw", "lt_gradient_grid_nfw_host",
-           "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_peak_probe"]
+           "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_mixed_last_sp_map", "lt_peak_probe"]
 
 
 class lt_mixed_params(ctypes.Structure):
@@ -99,6 +99,8 @@ def lib():
         L.lt_mixed_last_stats.restype = ci
         L.lt_mixed_last_flags.argtypes = [vp, ci, ci, ci, vp, vp]
         L.lt_mixed_last_flags.restype = ci
+        L.lt_mixed_last_sp_map.argtypes = [vp, ci, ci, ci, vp, vp]
+        L.lt_mixed_last_sp_map.restype = ci
         L.lt_peak_probe.argtypes = [ci, ci, ctypes.POINTER(cd), vp]
         L.lt_peak_probe.restype = ci
         _lib = L
@@ -113,6 +115,16 @@ def _check(rc, where):
 def _stream(stream):
     s = torch.cuda.current_stream() if stream is None else stream
     return ctypes.c_void_p(s.cuda_stream)
+
+
+def _keep(stream, *tensors):
+    """A tensor this binding allocated (or a contiguous copy it made) on the current stream and hands to kernels enqueued
+    on another `stream` must not go back to the caching allocator's pool before those kernels have run: record the use."""
+    if stream is None or stream == torch.cuda.current_stream():
+        return
+    for t in tensors:
+        if isinstance(t, torch.Tensor) and t.is_cuda:
+            t.record_stream(stream)
 
 
 def _lenses_dev(lenses, cols=7):
@@ -195,6 +207,7 @@ def lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None,
                              ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
                              workspace.numel(), _stream(stream))
     _check(rc, _fn)
+    _keep(stream, lenses, workspace, out)
     return out
 
 
@@ -220,6 +233,7 @@ def lt_gradient_grid_host(h_lenses, x_min, y_min, dx, nx, ny, mode, h_out, works
                              ctypes.c_void_p(h_out.data_ptr()), ctypes.c_void_p(workspace.data_ptr()),
                              workspace.numel(), _stream(stream))
     _check(rc, _fn)
+    _keep(stream, workspace)
     return h_out
 
 
@@ -245,6 +259,7 @@ def lt_gradient_points(lenses, points, out=None, workspace=None, stream=None, _f
                              ctypes.c_void_p(out.data_ptr() if n else None),
                              ctypes.c_void_p(workspace.data_ptr()), workspace.numel(), _stream(stream))
     _check(rc, _fn)
+    _keep(stream, lenses, points, workspace, out)
     return out
 
 
@@ -284,6 +299,7 @@ def lt_mixed_rule(sp_map, x_min, y_min, dx, centres, mixed=None, workspace=None,
                              ctypes.c_void_p(flags.data_ptr()), ctypes.c_void_p(workspace.data_ptr()), workspace.numel(),
                              _stream(stream))
     _check(rc, "lt_mixed_rule")
+    _keep(stream, centres, workspace, flags)
     return flags, workspace
 
 
@@ -310,6 +326,7 @@ def lt_find_images(grad, x_min, y_min, dx, dls_dos, sources, max_hits=1 << 16, h
                               ctypes.c_void_p(hits.data_ptr()), int(max_hits), ctypes.c_void_p(n_hits.data_ptr()),
                               _stream(stream))
     _check(rc, "lt_find_images")
+    _keep(stream, sources, hits, n_hits)
     return hits, n_hits
 
 
@@ -343,6 +360,7 @@ def lt_source_barycentres(theta, alpha, offsets, dls_dos, out=None, stream=None)
                                      ctypes.c_void_p(offsets.data_ptr()), n_sys, float(dls_dos),
                                      ctypes.c_void_p(out.data_ptr() if n_sys else None), _stream(stream))
     _check(rc, "lt_source_barycentres")
+    _keep(stream, theta, alpha, offsets, out)
     return out
 
 
@@ -369,6 +387,7 @@ def lt_chi2(theta_obs, sigma, offsets, hits, n_hits, terms=None, result=None, st
                        ctypes.c_void_p(terms.data_ptr() if n_img else None), ctypes.c_void_p(result.data_ptr()),
                        _stream(stream))
     _check(rc, "lt_chi2")
+    _keep(stream, theta_obs, sigma, offsets, hits, n_hits, terms, result)
     return result, terms
 
 
@@ -400,6 +419,14 @@ def lt_mixed_last_flags(workspace, n_lens, nx, ny, stream=None):
     out = torch.empty((ny, nx), dtype=torch.uint8, device=workspace.device)
     _check(lib().lt_mixed_last_flags(ctypes.c_void_p(workspace.data_ptr()), int(n_lens), int(nx), int(ny),
                                      ctypes.c_void_p(out.data_ptr()), _stream(stream)), "lt_mixed_last_flags")
+    return out
+
+
+def lt_mixed_last_sp_map(workspace, n_lens, nx, ny, stream=None):
+    """The single precision map ([ny, nx, 2] float32) the last LT_MIXED call on this workspace evaluated its rule on."""
+    out = torch.empty((ny, nx, 2), dtype=torch.float32, device=workspace.device)
+    _check(lib().lt_mixed_last_sp_map(ctypes.c_void_p(workspace.data_ptr()), int(n_lens), int(nx), int(ny),
+                                      ctypes.c_void_p(out.data_ptr()), _stream(stream)), "lt_mixed_last_sp_map")
     return out
 
 

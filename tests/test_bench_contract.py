@@ -19,7 +19,7 @@ def _run(extra, env=None):
     return r.stdout.strip()
 
 
-@pytest.mark.parametrize("extra,workload", [([], "cfg1_1024x1024_100"), (["--model", "sie"], "sie_paper_6730x6730_702"),
+@pytest.mark.parametrize("extra,workload", [([], "cfg3_4096x4096_1000"), (["--config", "1"], "cfg1_1024x1024_100"), (["--model", "sie"], "sie_paper_6730x6730_702"),
                                             (["--model", "nfw"], "nfw_512x512_64_n2048")])
 def test_reference_arm_line(extra, workload):
     out = _run(extra)
@@ -47,26 +47,51 @@ def test_reference_arm_other_ranks_are_silent():
 
 @pytest.mark.gpu
 def test_our_arm_line_on_the_gpu():
-    """The line bench.py prints for our arm carries every key of the contract (value, e2e with its byte counts,
-    gpu_launches, clocks, roofline with bound / achieved / peak / frac / traffic, cpu_baseline)."""
+    """The line bench.py prints for our arm, with its defaults: the largest single-GPU configuration, every key of the
+    contract (value, e2e with its byte counts, gpu_launches, clocks, roofline with bound / achieved / peak / frac /
+    traffic, cpu_baseline), the other modes, the other configs, and per mode the parity against the oracle with its
+    tolerance."""
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "3", "--warmup", "3", "--cpu-seconds", "0.5"],
-                       capture_output=True, text=True, timeout=900)
+                       capture_output=True, text=True, timeout=1500)
     assert r.returncode == 0, r.stderr
     lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
     assert len(lines) == 1
     d = json.loads(lines[0])
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
-              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline",
+              "modes", "configs", "parity"):
         assert k in d, k
     assert d["metric"] == "lens_pixel_gradient_evals_per_s" and d["dtype"] == "f64" and d["scaling"] == "weak"
-    assert d["config"]["workload"] == "cfg1_1024x1024_100" and d["vs_baseline"] is None
+    assert d["config"]["workload"] == "cfg3_4096x4096_1000" and d["vs_baseline"] is None
     assert d["value"] > 1e10 and d["gpu_launches"] >= 2 * d["steps"]
     e = d["e2e"]
-    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 100 * 56 and e["d2h_bytes_per_step"] == 1024 * 1024 * 16
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 1000 * 56 and e["d2h_bytes_per_step"] == 4096 * 4096 * 16
     rf = d["roofline"]
     assert rf["bound"] == "alu" and rf["unit"] == "TFLOP/s" and abs(rf["frac"] - rf["achieved"] / rf["peak"]) < 1e-12
-    assert rf["traffic"] is not None and 0 < rf["frac"] < 1
+    assert 0 < rf["frac"] < 1 and 0 < rf["executed"]["frac_of_floor"] < 1
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
     assert set(d["modes"]) == {"fp64", "fp32", "mixed"}
     assert "sm_mhz" in d["clocks"] and "reasons" in d["clocks"]
+    assert set(d["configs"]) == {"cfg1_1024x1024_100", "cfg2_2048x2048_500", "cfg4_stress_2048x2048_200",
+                                 "sie_paper_6730x6730_702"}
+    for block in [d] + list(d["configs"].values()):
+        for mode in ("fp64", "fp32", "mixed"):
+            p = block["parity"][mode]
+            assert p["pass"] and p["max_err_rel"] < p["tol"] and p["n_sampled"] >= 20000, (mode, p)
+        assert block["parity"]["mixed"]["flagged_bit_equal_to_fp64_mode"]
+    for name, cfg in d["configs"].items():
+        for mode in ("fp64", "fp32", "mixed"):
+            assert cfg[mode]["value"] > 1e10, (name, mode)
+
+
+@pytest.mark.gpu
+def test_strong_scaling_arm_on_one_gpu():
+    """--shard rows under one rank: the row-block arm runs, says so, and reports the same metric as strong scaling."""
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--shard", "rows", "--gather", "--config", "2",
+                        "--mode", "mixed", "--steps", "3", "--warmup", "3", "--no-extras"],
+                       capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr
+    d = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][0])
+    assert d["scaling"] == "strong" and d["config"]["parallelism"].startswith("rows/1")
+    assert d["shard"]["rows_per_rank"] == [2048] and len(d["shard"]["ms_per_rank"]) == 1 and d["value"] > 1e10

@@ -1,0 +1,154 @@
+"""Full-size parity through the C ABI, in the launch configuration bench.py times (pytest -m gpu):
+
+* every pixel of BASELINE configs 1 and 4 in all three modes against the long-double oracle (config 3, seven minutes of
+  oracle time, runs only with LT_FULLGRID_CFG3=1);
+* the mixed rule (a8: eq. 24-28, patches P:284) BIT-EXACT at sizes where lt_flag_kernel loops over several
+  tiles per CTA (more than 8 x 148 x 1024 = 1 212 416 pixels) and the recompute list is appended over several waves:
+  (i)  lt_mixed_rule on an ORACLE-made single precision map (the oracle's map rounded to fp32) against the oracle's rule;
+  (ii) the mask the end-to-end LT_MIXED call left behind against the oracle's rule evaluated on that call's own single
+       precision map (lt_mixed_last_sp_map; that map is checked against the oracle by the fp32 parity tests): the rule is
+       integer work on a given map and given lens centres, so this comparison is exact at any size;
+  counts (n_flagged, n_patch, n_eq25, n_eq28) bit-exact in both; a9: every flagged pixel carries the fp64 mode's bits.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1902_03252_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL_F64, TOL_F32 = 1e-12, 1e-5
+SIE_MIXED = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0)
+FLAG_SINGLE_ITERATION_PIXELS = 8 * 148 * 1024
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    from paper_1902_03252_b200 import lt
+    from oracle import lt_oracle as O, lt_oracle_sie as S
+    lt.lib()
+    return torch, lt, O, S
+
+
+_ORACLE_MAPS = {}
+
+
+def _oracle_map(O, W):
+    """long-double oracle map of a workload, computed once per test session (config 4: ~20-40 s on 16 cores)"""
+    if W.name not in _ORACLE_MAPS:
+        _ORACLE_MAPS[W.name] = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny)
+    return _ORACLE_MAPS[W.name]
+
+
+def _grid_fn(lt, W):
+    return {5: lt.lt_gradient_grid_sie}.get(W.lenses.shape[1], lt.lt_gradient_grid)
+
+
+def _run(torch, lt, W, mode, mixed=None):
+    L = torch.from_numpy(W.lenses).cuda()
+    ws = lt.alloc_workspace(len(W.lenses), W.nx, W.ny, mode)
+    out = _grid_fn(lt, W)(L, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, mixed=mixed, workspace=ws)
+    torch.cuda.synchronize()
+    rc, bad = lt.lt_last_status(ws)
+    assert rc == 0, (rc, bad)
+    return out, ws
+
+
+def _fullgrid(env, cfg):
+    torch, lt, O, S = env
+    W = workloads.make(cfg)
+    ref = _oracle_map(O, W)
+    s = np.abs(ref).reshape(-1, 2).max(axis=0)
+    res = {}
+    for mode, name in ((lt.LT_FP64, "fp64"), (lt.LT_FP32, "fp32"), (lt.LT_MIXED, "mixed")):
+        out = _run(torch, lt, W, mode)[0].cpu().numpy().astype(np.float64)
+        e = np.abs(out - ref).reshape(-1, 2)
+        res[name] = ((e.max(axis=0) / s).max(), (np.sqrt((e ** 2).mean(axis=0)) / s).max())
+        del out, e
+    print(W.name, "every pixel vs long-double oracle:", " | ".join("%s max %.3e rms %.3e" % (k, v[0], v[1]) for k, v in res.items()))
+    assert res["fp64"][0] < TOL_F64 and res["fp32"][0] < TOL_F32 and res["mixed"][0] < TOL_F32
+
+
+@pytest.mark.parametrize("cfg", [1, 4])
+def test_every_pixel_against_the_oracle(env, cfg):
+    _fullgrid(env, cfg)
+
+
+@pytest.mark.skipif(os.environ.get("LT_FULLGRID_CFG3") != "1", reason="~7 minutes of oracle time; set LT_FULLGRID_CFG3=1")
+def test_every_pixel_against_the_oracle_cfg3(env):
+    _fullgrid(env, 3)
+
+
+def _rule_catalogue(S, W):
+    return S.as_rule_catalogue(W.lenses) if W.lenses.shape[1] == 5 else W.lenses
+
+
+def _counts(flags):
+    return {"n_flagged": int((flags != 0).sum()), "n_patch": int(((flags & 1) != 0).sum()),
+            "n_eq25": int(((flags & 2) != 0).sum()), "n_eq28": int(((flags & 4) != 0).sum())}
+
+
+def test_rule_kernels_on_an_oracle_made_map_config4_full_size(env):
+    """(i) at 2048 x 2048 = 4.2 M pixels: every CTA of lt_flag_kernel iterates 3-4 times"""
+    torch, lt, O, S = env
+    W = workloads.make(4)
+    assert W.nx * W.ny > FLAG_SINGLE_ITERATION_PIXELS
+    sp = np.ascontiguousarray(_oracle_map(O, W).astype(np.float32))
+    expect = O.mixed_flags(sp, W.lenses, W.x_min, W.y_min, W.dx, mixed=O.DEFAULT_MIXED)
+    centres = torch.from_numpy(np.ascontiguousarray(W.lenses[:, [0, 1, 6]])).cuda()
+    flags, ws = lt.lt_mixed_rule(torch.from_numpy(sp).cuda(), W.x_min, W.y_min, W.dx, centres)
+    torch.cuda.synchronize()
+    assert np.array_equal(flags.cpu().numpy(), expect)
+    assert lt.lt_mixed_last_stats(ws) == _counts(expect)
+
+
+def test_rule_kernels_on_an_oracle_made_map_sie_window(env):
+    """(i) on a 2048 x 2048 window of the paper-like benchmark grid around the first cluster halo, paper constants at the
+    paper's pixel size: both patch sizes, the critical-line bands and plain SP regions are inside the window"""
+    torch, lt, O, S = env
+    W = workloads.make_sie("paper")
+    i0 = int(round((W.lenses[0, 0] - W.x_min) / W.dx)) - 1024
+    j0 = int(round((W.lenses[0, 1] - W.y_min) / W.dx)) - 1024
+    i0, j0 = min(max(i0, 0), W.nx - 2048), min(max(j0, 0), W.ny - 2048)
+    W = W._replace(x_min=W.x_min + i0 * W.dx, y_min=W.y_min + j0 * W.dx, nx=2048, ny=2048)
+    sp = np.ascontiguousarray(S.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny).astype(np.float32))
+    cat = _rule_catalogue(S, W)
+    expect = O.mixed_flags(sp, cat, W.x_min, W.y_min, W.dx, mixed=SIE_MIXED)
+    centres = torch.from_numpy(np.ascontiguousarray(cat[:, [0, 1, 6]])).cuda()
+    flags, ws = lt.lt_mixed_rule(torch.from_numpy(sp).cuda(), W.x_min, W.y_min, W.dx, centres, mixed=SIE_MIXED)
+    torch.cuda.synchronize()
+    c = _counts(expect)
+    assert np.array_equal(flags.cpu().numpy(), expect) and lt.lt_mixed_last_stats(ws) == c
+    assert 0 < c["n_patch"] < c["n_flagged"] < W.nx * W.ny            # the window exercises every branch of the rule
+    print("sie window: counts", c)
+
+
+@pytest.mark.parametrize("which", ["cfg2", "cfg3", "cfg4", "sie"])
+def test_end_to_end_mask_is_the_rule_on_the_calls_own_sp_map(env, which):
+    """(ii) at full size: 4.2 M (configs 2, 4), 16.8 M (config 3) and 45.3 M pixels (SIE benchmark)"""
+    torch, lt, O, S = env
+    W = workloads.make_sie("paper") if which == "sie" else workloads.make(int(which[3:]))
+    mixed = SIE_MIXED if which == "sie" else None
+    assert W.nx * W.ny > FLAG_SINGLE_ITERATION_PIXELS
+    m, ws = _run(torch, lt, W, lt.LT_MIXED, mixed=mixed)
+    flags = lt.lt_mixed_last_flags(ws, len(W.lenses), W.nx, W.ny).cpu().numpy()
+    sp = lt.lt_mixed_last_sp_map(ws, len(W.lenses), W.nx, W.ny).cpu().numpy()
+    stats = lt.lt_mixed_last_stats(ws)
+    expect = O.mixed_flags(sp, _rule_catalogue(S, W), W.x_min, W.y_min, W.dx, mixed=mixed or O.DEFAULT_MIXED)
+    assert np.array_equal(flags, expect)
+    assert stats == _counts(expect)
+    # the single precision map of the mixed call is the fp32 mode's map (which the parity tests compare with the oracle)
+    g32, _ = _run(torch, lt, W, lt.LT_FP32)
+    assert np.array_equal(sp, g32.cpu().numpy())
+    del g32
+    # a9: flagged pixels carry the fp64 mode's bits, the others the single precision value widened (R17)
+    g64, _ = _run(torch, lt, W, lt.LT_FP64)
+    f = torch.from_numpy(expect != 0).cuda()
+    assert bool(torch.equal(m[f], g64[f]))
+    assert bool(torch.equal(m[~f], torch.from_numpy(sp).cuda().double()[~f]))
+    print(W.name, "flagged fraction", stats["n_flagged"] / (W.nx * W.ny), stats)
