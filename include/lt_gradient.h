@@ -307,6 +307,36 @@ int lt_mixed_last_flags(const void* d_workspace, int n_lens, int nx, int ny, uns
  * centres alone.  Asynchronous on cuda_stream. */
 int lt_mixed_last_sp_map(const void* d_workspace, int n_lens, int nx, int ny, float* d_sp_out, void* cuda_stream);
 
+/*
+ * The paper's accuracy criterion on a pair of maps (section 3.2): a single precision gradient is accurate
+ * enough where |err_i| <= dx / (4 M_i), M_i = dx / |dx - delta_i| the magnification along axis i (eq. 24, 26, P:298-310;
+ * delta_i from the DOUBLE precision map; forward neighbour in the first column / row, delta = 0 along an axis of extent 1).
+ * This is the measurement behind the constants of the mixed rule (M_max = (dx/4) / E_SP = 3.26 for the paper's SIE error
+ * model), which "has to be computed for each model independently": SURVEY 8(f) NEXT-2.
+ *   d_sp_map      nx*ny*2 floats  (e.g. lt_mixed_last_sp_map, or an LT_FP32 map)
+ *   d_dp_map      nx*ny*2 doubles (an LT_FP64 map of the same grid)
+ *   d_centres     n_centres * 3 doubles (x, y, unused) or NULL: lens centres for the error-by-distance table
+ *   d_flags       nx*ny bytes, the rule's mask (lt_mixed_last_flags: bit 0 = centre patch) or NULL
+ *   d_violation   nx*ny bytes out or NULL: bit 0 / bit 1 = component 1 / 2 exceeds its budget
+ *   d_result      one lt_audit_result in DEVICE memory (8-byte aligned), zeroed and filled by the call
+ * Asynchronous on cuda_stream; read the result with lt_rule_audit_result.  max_err_by_distance[k]: largest |SP - DP|
+ * (worse component, arcsec) among the pixels whose Chebyshev distance in pixels to the nearest centre lies in
+ * [0,1) [1,2) [2,4) [4,8) [8,16) [16,32) [32,64) [64,128) [128,inf): the table form of Fig. 9; 0 = empty bin.
+ */
+#define LT_AUDIT_BINS 9
+typedef struct {
+  long long n_pixels, n_violating, n_violating_flagged, n_violating_missed, n_flagged;
+  double max_err, max_err_in_patch, max_err_outside_patch;    /* arcsec; patch = bit 0 of d_flags */
+  double max_err_by_distance[LT_AUDIT_BINS];
+  double implied_m_max, implied_m_max_outside_patch;          /* (dx/4) / max_err...: filled by lt_rule_audit_result */
+} lt_audit_result;
+int lt_rule_audit(const float* d_sp_map, const double* d_dp_map, double x_min, double y_min, double dx, int nx, int ny,
+                  const double* d_centres, int n_centres, const unsigned char* d_flags, unsigned char* d_violation,
+                  lt_audit_result* d_result, void* cuda_stream);
+/* Copies the result of lt_rule_audit to the host (synchronises cuda_stream) and fills the two implied_m_max fields
+ * (M_max = (dx / 4) / E_SP; inf when the error is 0). */
+int lt_rule_audit_result(const lt_audit_result* d_result, double dx, void* cuda_stream, lt_audit_result* h_out);
+
 /* FMA-chain microbenchmarks used by bench.py to confirm the FP64 / FP32 peaks on the device in the same run
  * (SURVEY 8(d)): runs `iters` dependent-free FMAs per thread on a full grid; returns achieved FLOP/s in *flops_out
  * (2 flops per FMA).  Synchronises.  which: 0 = fp64, 1 = fp32. */

@@ -39,19 +39,22 @@ def up_to_date():
     return all(os.path.getmtime(os.path.join(HERE, d)) <= t for d in deps())
 
 
-def build(force=False, verbose=False):
-    if not force and up_to_date():
+def build(force=False, verbose=False, defines=(), out=None):
+    """defines / out: an experimental build (-D<name> ...) written to another path; lt.py loads it when the environment
+    variable LT_GRADIENT_LIB names it.  The default build takes neither."""
+    lib = out or LIB
+    if not force and not defines and out is None and up_to_date():
         return LIB
-    tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
+    tmp = lib + ".tmp%d" % os.getpid()
+    cmd = [nvcc()] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
           [os.path.join(HERE, s) for s in SOURCES]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":

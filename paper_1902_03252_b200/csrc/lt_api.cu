@@ -15,6 +15,7 @@
 #include "lt_mixed.cuh"
 #include "lt_images.cuh"
 #include "lt_chi2.cuh"
+#include "lt_audit.cuh"
 
 static_assert(sizeof(lt_lens) == sizeof(LtRawLens), "lt_lens and LtRawLens must have the same layout");
 static_assert(sizeof(lt_image_hit) == sizeof(LtImageHit) && sizeof(LtImageHit) == 32, "lt_image_hit layout");
@@ -40,6 +41,9 @@ Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
 thread_local int g_launches = 0;                                      // kernels launched by the last entry-point call
 
+#ifndef LT_PPT32_PACKED
+#define LT_PPT32_PACKED 4          // pixels per thread of the packed fp32 grid kernel (4 or 8)
+#endif
 constexpr int kDefaultChunk64 = 256;   // 32 KB of fp64 records per CTA
 constexpr int kDefaultChunk32 = 1024;  // 64 KB of fp32 records per CTA
 constexpr size_t kAlign = 256;
@@ -186,7 +190,7 @@ int pick_chunk(K kernel, int n_lens, int wanted, size_t rec_bytes, const DeviceI
 
 // pixels per thread: the largest of the candidates that still gives every SM about two tiles
 int pick_ppt(int wanted, int max_ppt, int nx, int ny, const DeviceInfo& d) {
-  if (wanted == 1 || wanted == 2 || wanted == 4) return wanted <= max_ppt ? wanted : max_ppt;
+  if (wanted == 1 || wanted == 2 || wanted == 4 || wanted == 8) return wanted <= max_ppt ? wanted : max_ppt;
   int ppt = max_ppt;
   while (ppt > 1) {
     const long long tiles = (long long)((nx + 32 * ppt - 1) / (32 * ppt)) * ((ny + LT_TILE_H - 1) / LT_TILE_H);
@@ -321,8 +325,13 @@ int launch_f32(const typename Rec64<M>::type* l64, const typename Rec32<M>::type
   // 4 pixels per thread at <= 80 registers (3 CTAs per SM): with a tighter register budget the compiler reloads the
   // constants inside the loop and the kernel, which is bound by issue slots, loses 10 %
   KernelEvents ke(st, hook);
-  return launch_waves(pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d), a,
+  return launch_waves(pick_ppt(g_tuning.ppt32, M::kPacked32 ? LT_PPT32_PACKED : 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
+                        if constexpr (M::kPacked32 && LT_PPT32_PACKED == 8) {   // four pixel pairs per thread
+                          if (ppt == 8)
+                            return out_wide ? launch_f32_ppt<M, 8, 2, true>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident)
+                                            : launch_f32_ppt<M, 8, 2, false>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
+                        }
                         if (out_wide) {      // mixed mode: the kernel variant that also stores the widened value
                           switch (ppt) {
                             case 1: return launch_f32_ppt<M, 1, 6, true>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
@@ -857,6 +866,44 @@ int lt_mixed_last_sp_map(const void* d_workspace, int n_lens, int nx, int ny, fl
   const Layout L = make_layout(n_lens, (long long)nx * ny, true);
   LT_CUDA(cudaMemcpyAsync(d_sp_out, (const unsigned char*)d_workspace + L.sp, (size_t)nx * ny * sizeof(float2),
                           cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+  return LT_OK;
+}
+
+int lt_rule_audit(const float* d_sp_map, const double* d_dp_map, double x_min, double y_min, double dx, int nx, int ny,
+                  const double* d_centres, int n_centres, const unsigned char* d_flags, unsigned char* d_violation,
+                  lt_audit_result* d_result, void* cuda_stream) {
+  static_assert(sizeof(lt_audit_result) == sizeof(LtAuditResult), "lt_audit_result layout");
+  if (!sizes_ok(0, nx, ny) || n_centres < 0) return LT_ERR_BAD_SIZE;
+  if (!d_sp_map || !d_dp_map || !d_result || (n_centres > 0 && !d_centres)) return LT_ERR_NULL_POINTER;
+  if (!(isfinite(x_min) && isfinite(y_min) && isfinite(dx)) || !(dx > 0.0)) return LT_ERR_BAD_GRID;
+  if (((uintptr_t)d_sp_map & 7) || ((uintptr_t)d_dp_map & 15) || ((uintptr_t)d_result & 7) || ((uintptr_t)d_centres & 7))
+    return LT_ERR_MISALIGNED;
+  DeviceInfo dev;
+  const int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LT_CUDA(cudaMemsetAsync(d_result, 0, sizeof(lt_audit_result), st));
+  const long long n_pix = (long long)nx * ny;
+  long long blocks = (n_pix + 255) / 256;
+  if (blocks > (long long)dev.sms * 8) blocks = (long long)dev.sms * 8;
+  lt_rule_audit_kernel<<<(int)blocks, 256, 0, st>>>(reinterpret_cast<const float2*>(d_sp_map),
+                                                    reinterpret_cast<const double2*>(d_dp_map), x_min, y_min, dx, nx, ny,
+                                                    d_centres, n_centres, d_flags, d_violation,
+                                                    reinterpret_cast<LtAuditResult*>(d_result));
+  LT_CUDA(cudaGetLastError());
+  ++g_launches;
+  return LT_OK;
+}
+
+int lt_rule_audit_result(const lt_audit_result* d_result, double dx, void* cuda_stream, lt_audit_result* h_out) {
+  if (!d_result || !h_out) return LT_ERR_NULL_POINTER;
+  if (!(dx > 0.0)) return LT_ERR_BAD_GRID;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  LT_CUDA(cudaMemcpyAsync(h_out, d_result, sizeof(lt_audit_result), cudaMemcpyDeviceToHost, st));
+  LT_CUDA(cudaStreamSynchronize(st));
+  h_out->implied_m_max = dx / 4.0 / h_out->max_err;                                /* P:284 */
+  h_out->implied_m_max_outside_patch = dx / 4.0 / h_out->max_err_outside_patch;
   return LT_OK;
 }
 

@@ -13,7 +13,9 @@
 #include <cuda_runtime.h>
 #include "lt_pack.cuh"
 
+#ifndef LT_WARPS_PER_CTA
 #define LT_WARPS_PER_CTA 8
+#endif
 #define LT_THREADS (32 * LT_WARPS_PER_CTA)
 #define LT_TILE_H LT_WARPS_PER_CTA
 #define LT_PRECOMPUTE_THREADS 128
@@ -93,6 +95,20 @@ __device__ __forceinline__ void lt_copy16(void* dst, const void* src, int count)
   for (int w = threadIdx.x; w < count; w += blockDim.x) d[w] = s[w];
 }
 
+template <bool C, class A, class B> struct LtSelect { typedef A type; };
+template <class A, class B> struct LtSelect<false, A, B> { typedef B type; };
+// global (tau, phi) entries -> the shared structure-of-arrays copy the packed fp32 body reads (lt_math.cuh)
+__device__ __forceinline__ void lt_stage_tables2(LtTables2* dst, const LtTables<float>* __restrict__ src) {
+  for (int k = threadIdx.x; k < 2 * LT_ATAN_B + 1; k += blockDim.x) {
+    dst->at_tau[k] = src->at[k][0];
+    dst->at_phi[k] = src->at[k][1];
+  }
+  for (int k = threadIdx.x; k < 2 * LT_ATANH_B + 1; k += blockDim.x) {
+    dst->ah_tau[k] = src->ah[k][0];
+    dst->ah_K[k] = src->ah[k][1];
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ fp64 grid kernel
 // a2 pixel coordinate (x_min + i*dx, product and sum rounded separately, exactly as the API states it), a3-a6 per
 // lens (the model's interact_sky), a7 one double2 store per pixel.
@@ -170,11 +186,17 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
   extern __shared__ __align__(16) unsigned char lt_smem[];
   typedef typename M::template Rec<float>::type Rec;
   typedef typename M::template Rec<double>::type Rec64;
-  __shared__ LtTables<float> tab;
+  constexpr int TILE_W = 32 * PPT;
+  constexpr bool PACK = M::kPacked32 && !M::kSkyFrame32 && (PPT % 2 == 0);
+  __shared__ typename LtSelect<PACK, LtTables2, LtTables<float>>::type tab;
   Rec* sl = reinterpret_cast<Rec*>(lt_smem);
   lt_grid_dependency_wait();
-  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));   // visible after the first __syncthreads of the chunk loop
-  constexpr int TILE_W = 32 * PPT;
+  // the tables become visible with the first __syncthreads of the chunk loop
+  if constexpr (PACK) {
+    lt_stage_tables2(reinterpret_cast<LtTables2*>(&tab), tables);
+  } else if (M::kTables) {
+    lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  }
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   // in-tile offsets from the tile centre, in pixels (exact in fp32)
   const float fdx = (float)dx;
@@ -190,10 +212,13 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
     const double cx = x_min + ((double)(tx * TILE_W) + 0.5 * (double)(TILE_W - 1)) * dx;
     const double cy = y_min + ((double)(ty * LT_TILE_H) + 0.5 * (double)(LT_TILE_H - 1)) * dx;
     float G1[PPT], G2[PPT];
+    lt_f2 H1[(PPT + 1) / 2], H2[(PPT + 1) / 2];      // PACK: the accumulators of pixel pairs (2p, 2p + 1)
 #pragma unroll
     for (int p = 0; p < PPT; ++p) {
       G1[p] = 0.f;
       G2[p] = 0.f;
+      H1[p / 2] = lt2(0.f);
+      H2[p / 2] = lt2(0.f);
     }
     for (int base = 0; base < n_lens; base += chunk) {
       const int cnt = min(chunk, n_lens - base);
@@ -205,14 +230,8 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
           F.x0 = (float)(cx - D.x0);
           F.y0 = (float)(cy - D.y0);
         } else {                                    // (scaled) lens-frame position of the tile centre
-#ifdef LT_V_X0
           F.x0 = (float)fma(cx, D.cx, fma(cy, D.sx, -D.x0));
           F.y0 = (float)fma(-cx, D.sy, fma(cy, D.cy, -D.y0));
-#else
-          const double d1 = cx - D.x0, d2 = cy - D.y0;
-          F.x0 = (float)fma(d1, D.cx, d2 * D.sx);
-          F.y0 = (float)fma(-d1, D.sy, d2 * D.cy);
-#endif
         }
         sl[k] = F;
       }
@@ -226,6 +245,16 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
 #pragma unroll
           for (int p = 0; p < PPT; ++p)
             M::template interact_sky<float>(fmaf(il[p], fdx, L.x0), row, L, tab, G1[p], G2[p]);   // Alg. 1 l.3-14
+        } else if constexpr (PACK) {                  // two pixels of the thread per instruction (lt_math.cuh)
+          const float xr = fmaf(jl, L.sx, L.x0);
+          const float yr = fmaf(jl, L.cy, L.y0);
+#pragma unroll
+          for (int p = 0; p < PPT; p += 2) {
+            const lt_f2 il2 = lt2(il[p], il[p + 1]);
+            const lt_f2 x = lt2_fma(il2, lt2(L.cx), lt2(xr));
+            const lt_f2 y = lt2_fma(lt2_neg(il2), lt2(L.sy), lt2(yr));
+            M::interact_lens_x2(x, y, L, tab, H1[p / 2], H2[p / 2]);   // Alg. 1 l.7-14
+          }
         } else {
           const float xr = fmaf(jl, L.sx, L.x0);
           const float yr = fmaf(jl, L.cy, L.y0);
@@ -236,6 +265,13 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
             M::template interact_lens<float>(x, y, L, tab, G1[p], G2[p]);   // Alg. 1 l.7-14
           }
         }
+      }
+    }
+    if constexpr (PACK) {
+#pragma unroll
+      for (int p = 0; p < PPT; ++p) {
+        G1[p] = (p & 1) ? H1[p / 2].y : H1[p / 2].x;
+        G2[p] = (p & 1) ? H2[p / 2].y : H2[p / 2].x;
       }
     }
     if (j < ny) {

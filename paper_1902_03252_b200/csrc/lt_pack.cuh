@@ -17,7 +17,10 @@ LT_HD bool lt_lens_valid(const LtRawLens& r) {
   return fin && r.e >= 0.0 && r.e < 1.0 && r.rcore > 0.0 && r.rcut > r.rcore;
 }
 
-// fp64 record.  x0, y0 = lens centre; dxc, dxs = dx cos Phi, dx sin Phi.
+// fp64 record.  The translation of Alg. 1 l.3-4 is folded into the rotation of l.5-6: X = cx (t1 - xc) + sx (t2 - yc) =
+// cx t1 + sx t2 - X0 with X0 = cx xc + sx yc formed once per lens (two FMAs per coordinate and pixel instead of a
+// subtraction and an FMA; the rounding of X0, 1e-16 of |theta_c|, is to the lens-frame coordinate what the rounding of
+// the pixel coordinate itself is).
 LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
   double s, c;
   sincos(r.phi, &s, &c);
@@ -33,14 +36,9 @@ LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
   L.sx = qf * s;
   L.cy = rf * c;
   L.sy = rf * s;
-#ifdef LT_V_X0
   // scaled lens-frame coordinates of the sky origin, negated: X = cx t1 + sx t2 - X0, Y = cy t2 - sy t1 - Y0
   L.x0 = fma(L.cx, r.x, L.sx * r.y);
   L.y0 = fma(L.cy, r.y, -(L.sy * r.x));
-#else
-  L.x0 = r.x;
-  L.y0 = r.y;
-#endif
   L.Kc = (ome * r.rcore * rf) * (ome * r.rcore * rf);  // q^2 s_c^2 / f^2
   L.Kt = (ome * r.rcut * rf) * (ome * r.rcut * rf);
   L.sc = sc * rf;
@@ -159,6 +157,13 @@ struct LtDpieModel {
   template <class T> struct Row { T d2sx, d2cy; };
   static constexpr bool kTables = true;
   static constexpr bool kSkyFrame32 = false;
+  static constexpr bool kPacked32 = true;      // the fp32 grid kernel evaluates two pixels per instruction (interact_lens_x2)
+#if defined(__CUDACC__)
+  static __device__ __forceinline__ void interact_lens_x2(const lt_f2 X, const lt_f2 Y, const LtLens<float>& L,
+                                                          const LtTables2& tab, lt_f2& G1, lt_f2& G2) {
+    lt_dpie_interact_x2(X, Y, L, tab, G1, G2);
+  }
+#endif
   static LT_HD bool valid(const Raw& r) { return lt_lens_valid(r); }
   static LT_HD void pack(const Raw& r, LtLens<double>& L) { lt_pack_lens(r, L); }
   static LT_HD void poison(LtLens<double>& L) { lt_poison_lens(L); }
@@ -180,7 +185,6 @@ struct LtDpieModel {
     interact_lens<T, GRID>(X, Y, L, tab, G1, G2);
   }
   // the same from the absolute sky coordinates (t1, t2) of the pixel: what the fp64 kernels call
-#ifdef LT_V_X0
   template <class T> static LT_HD Row<T> row_abs(const T t2, const LtLens<T>& L) {
     return Row<T>{lt_fma(t2, L.sx, -L.x0), lt_fma(t2, L.cy, -L.y0)};
   }
@@ -188,19 +192,13 @@ struct LtDpieModel {
   static LT_HD void interact_abs(const T t1, const Row<T>& r, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
     interact_sky<T, GRID>(t1, r, L, tab, G1, G2);
   }
-#else
-  template <class T> static LT_HD Row<T> row_abs(const T t2, const LtLens<T>& L) { return row<T>(t2 - L.y0, L); }
-  template <class T, bool GRID = false>
-  static LT_HD void interact_abs(const T t1, const Row<T>& r, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
-    interact_sky<T, GRID>(t1 - L.x0, r, L, tab, G1, G2);
-  }
-#endif
 };
 struct LtSieModel {
   typedef LtRawSie Raw;
   template <class T> struct Rec { typedef LtSieLens<T> type; };
   static constexpr bool kTables = false;
   static constexpr bool kSkyFrame32 = true;
+  static constexpr bool kPacked32 = false;
   static LT_HD bool valid(const Raw& r) { return lt_sie_valid(r); }
   static LT_HD void pack(const Raw& r, LtSieLens<double>& L) { lt_pack_sie(r, L); }
   static LT_HD void poison(LtSieLens<double>& L) { lt_poison_sie(L); }
@@ -226,6 +224,7 @@ struct LtNfwModel {
   template <class T> struct Rec { typedef LtNfwLens<T> type; };
   static constexpr bool kTables = true;
   static constexpr bool kSkyFrame32 = true;
+  static constexpr bool kPacked32 = false;
   static LT_HD bool valid(const Raw& r) { return lt_nfw_valid(r); }
   static LT_HD void pack(const Raw& r, LtNfwLens<double>& L) { lt_pack_nfw(r, L); }
   static LT_HD void poison(LtNfwLens<double>& L) { lt_poison_nfw(L); }

@@ -17,14 +17,15 @@ LT_OK = 0
 LT_ERR_BAD_LENS_PARAMS = -9
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "liblt_gradient.so")
+# LT_GRADIENT_LIB: another build of the same library (csrc/build.py: defines / out) -- for kernel experiments
+_LIB_PATH = os.environ.get("LT_GRADIENT_LIB") or os.path.join(_HERE, "liblt_gradient.so")
 
 SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defaults", "lt_workspace_bytes",
            "lt_gradient_grid", "lt_gradient_points", "lt_host_workspace_bytes", "lt_gradient_grid_host",
            "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images", "lt_mixed_rule",
            "lt_source_barycentres", "lt_chi2",
            "lt_gradient_grid_nfw", "lt_gradient_points_nfw", "lt_gradient_grid_nfw_host",
-           "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_mixed_last_sp_map", "lt_peak_probe"]
+           "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_mixed_last_sp_map", "lt_rule_audit", "lt_rule_audit_result", "lt_peak_probe"]
 
 
 class lt_mixed_params(ctypes.Structure):
@@ -35,6 +36,18 @@ class lt_mixed_params(ctypes.Structure):
 class lt_mixed_stats(ctypes.Structure):
     _fields_ = [("n_pixels", ctypes.c_longlong), ("n_flagged", ctypes.c_longlong), ("n_patch", ctypes.c_longlong),
                 ("n_eq25", ctypes.c_longlong), ("n_eq28", ctypes.c_longlong)]
+
+
+LT_AUDIT_BINS = 9
+AUDIT_BIN_EDGES_PX = (0, 1, 2, 4, 8, 16, 32, 64, 128)
+
+
+class lt_audit_result(ctypes.Structure):
+    _fields_ = [("n_pixels", ctypes.c_longlong), ("n_violating", ctypes.c_longlong),
+                ("n_violating_flagged", ctypes.c_longlong), ("n_violating_missed", ctypes.c_longlong),
+                ("n_flagged", ctypes.c_longlong), ("max_err", ctypes.c_double), ("max_err_in_patch", ctypes.c_double),
+                ("max_err_outside_patch", ctypes.c_double), ("max_err_by_distance", ctypes.c_double * LT_AUDIT_BINS),
+                ("implied_m_max", ctypes.c_double), ("implied_m_max_outside_patch", ctypes.c_double)]
 
 
 class LtError(RuntimeError):
@@ -101,6 +114,10 @@ def lib():
         L.lt_mixed_last_flags.restype = ci
         L.lt_mixed_last_sp_map.argtypes = [vp, ci, ci, ci, vp, vp]
         L.lt_mixed_last_sp_map.restype = ci
+        L.lt_rule_audit.argtypes = [vp, vp, cd, cd, cd, ci, ci, vp, ci, vp, vp, vp, vp]
+        L.lt_rule_audit.restype = ci
+        L.lt_rule_audit_result.argtypes = [vp, cd, vp, ctypes.POINTER(lt_audit_result)]
+        L.lt_rule_audit_result.restype = ci
         L.lt_peak_probe.argtypes = [ci, ci, ctypes.POINTER(cd), vp]
         L.lt_peak_probe.restype = ci
         _lib = L
@@ -428,6 +445,38 @@ def lt_mixed_last_sp_map(workspace, n_lens, nx, ny, stream=None):
     _check(lib().lt_mixed_last_sp_map(ctypes.c_void_p(workspace.data_ptr()), int(n_lens), int(nx), int(ny),
                                       ctypes.c_void_p(out.data_ptr()), _stream(stream)), "lt_mixed_last_sp_map")
     return out
+
+
+def lt_rule_audit(sp_map, dp_map, x_min, y_min, dx, centres=None, flags=None, want_violation=False, stream=None):
+    """The paper's accuracy criterion |err_i| <= dx / (4 M_i) of a single precision map ([ny, nx, 2] float32
+    CUDA) against a double precision map ([ny, nx, 2] float64 CUDA).  centres: [n, 3] float64 CUDA or None; flags: the
+    rule's mask ([ny, nx] uint8 CUDA) or None.  Synchronises.  Returns (dict of lt_audit_result's fields, violation
+    map [ny, nx] uint8 CUDA or None)."""
+    if not (sp_map.is_cuda and sp_map.dtype == torch.float32 and sp_map.is_contiguous() and sp_map.dim() == 3):
+        raise TypeError("sp_map must be a contiguous CUDA float32 tensor [ny, nx, 2]")
+    if not (dp_map.is_cuda and dp_map.dtype == torch.float64 and dp_map.is_contiguous() and dp_map.shape == sp_map.shape):
+        raise TypeError("dp_map must be a contiguous CUDA float64 tensor of sp_map's shape")
+    ny, nx = sp_map.shape[0], sp_map.shape[1]
+    n = 0
+    if centres is not None:
+        centres = centres.reshape(-1, 3).contiguous()
+        n = centres.shape[0]
+    if flags is not None and not (flags.is_cuda and flags.dtype == torch.uint8 and flags.is_contiguous() and flags.numel() == nx * ny):
+        raise TypeError("flags must be a contiguous CUDA uint8 tensor [ny, nx]")
+    viol = torch.empty((ny, nx), dtype=torch.uint8, device=sp_map.device) if want_violation else None
+    d_res = torch.empty(ctypes.sizeof(lt_audit_result), dtype=torch.uint8, device=sp_map.device)
+    _check(lib().lt_rule_audit(ctypes.c_void_p(sp_map.data_ptr()), ctypes.c_void_p(dp_map.data_ptr()), float(x_min),
+                               float(y_min), float(dx), int(nx), int(ny),
+                               ctypes.c_void_p(centres.data_ptr() if n else None), n,
+                               ctypes.c_void_p(flags.data_ptr() if flags is not None else None),
+                               ctypes.c_void_p(viol.data_ptr() if viol is not None else None),
+                               ctypes.c_void_p(d_res.data_ptr()), _stream(stream)), "lt_rule_audit")
+    h = lt_audit_result()
+    _check(lib().lt_rule_audit_result(ctypes.c_void_p(d_res.data_ptr()), float(dx), _stream(stream), ctypes.byref(h)),
+           "lt_rule_audit_result")
+    out = {name: getattr(h, name) for name, _ in lt_audit_result._fields_ if name != "max_err_by_distance"}
+    out["max_err_by_distance"] = list(h.max_err_by_distance)
+    return out, viol
 
 
 def lt_peak_probe(which, iters=1 << 16, stream=None):
