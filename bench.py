@@ -61,11 +61,15 @@ PAPER_V100_SIE = {"fp64": 6.9e10, "mixed": 8.2e10}
 # lanes per SM behind the "alu" peaks (paper's Table 1 convention: 2 ops/cycle x clock x lanes)
 LANES = {"fp64": 64, "fp32": 128, "mixed": 64}
 KERNEL_NAME = {"fp64": "lt_grad_f64_kernel", "fp32": "lt_grad_f32_kernel", "mixed": "lt_grad_list_f64_kernel"}
-# Instructions per interaction of the 4-pixel inner loops, counted in the SASS of the library as built at HEAD
-# (cuobjdump -sass; profiles/README.md says how).  fp64 / mixed: FP64-pipe instructions, each holding an SMSP's 16-lane
-# FP64 pipe for 2 cycles; fp32: all instructions, one issue slot each.
-INSTR_PER_INTERACTION = {("dpie", "fp64"): 61.75, ("dpie", "mixed"): 64.0, ("dpie", "fp32"): 62.75,
-                         ("sie", "fp64"): 12.75, ("sie", "mixed"): 15.75}
+# Cycles per interaction that the inner loops of the library as built at HEAD need on the pipe that bounds them, from
+# the SASS (cuobjdump -sass; profiles/README.md says how): (pipe, instructions of that pipe per interaction, cycles each
+# holds the SMSP's pipe for one warp).  fp64 / mixed: FP64 instructions, 16 lanes, 2 cycles; fp32: the FMA pipe takes a
+# packed FFMA2 / FMUL2 / FADD2 for 2 cycles (32 lanes, two results each); SIE fp32: one MUFU.RSQ per interaction on the
+# 4-lane XU, 8 cycles -- above its 7.75 FMA-pipe cycles.
+PIPE_FLOOR = {("dpie", "fp64"): ("fp64", 60.5, 2.0), ("dpie", "mixed"): ("fp64", 60.5, 2.0),
+              ("dpie", "fp32"): ("fp32 fma (packed pairs)", 20.25, 2.0),
+              ("sie", "fp64"): ("fp64", 12.75, 2.0), ("sie", "mixed"): ("fp64", 12.75, 2.0),
+              ("sie", "fp32"): ("xu (MUFU.RSQ)", 1.0, 8.0)}
 # dram__bytes_{read,write}.sum per launch of the dominant kernels, written by the ncu recipe of profiles/README.md
 NCU_TRAFFIC_JSON = os.path.join(ROOT, "profiles", "ncu_traffic.json")
 MIXED_SIE = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0)   # the paper's rule at its own pixel size; cluster-scale = b0 >= 1"
@@ -449,13 +453,12 @@ class Bench:
     # ---- roofline of one measurement
     def executed(self, model, mode, ms_k, units):
         """The same launch against the instruction floor of the pipe that bounds it."""
-        per = INSTR_PER_INTERACTION.get((model, mode))
-        if per is None:
+        entry = PIPE_FLOOR.get((model, mode))
+        if entry is None:
             return None
-        cycles = per * (2.0 if mode != "fp32" else 1.0)
-        floor = self.sms * 4 * self.sm_max * 1e6 * 32 / cycles          # interactions per second at 100 % of the pipe
-        return {"instructions_per_interaction": per,
-                "pipe": "fp64 (2 cycles per warp instruction)" if mode != "fp32" else "issue slots (1 per warp instruction)",
+        pipe, per, cyc = entry
+        floor = self.sms * 4 * self.sm_max * 1e6 * 32 / (per * cyc)     # interactions per second at 100 % of the pipe
+        return {"pipe": pipe, "instructions_per_interaction": per, "cycles_per_instruction": cyc,
                 "floor_interactions_per_s": floor, "frac_of_floor": units / (ms_k * 1e-3) / floor}
 
     def roofline(self, W, m, mode):

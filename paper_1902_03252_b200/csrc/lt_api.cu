@@ -35,15 +35,12 @@ thread_local int g_last_cuda_error = 0;
 // that races lt_set_tuning sees every knob either old or new (the knobs are independent of one another)
 struct Tuning {
   std::atomic<int> ppt64{0}, ppt32{0}, chunk64{0}, chunk32{0}, ctas_per_sm{0}, single_launch{0}, staged_host_output{0},
-      points_per_thread{0}, no_dependent_launch{0};
+      points_per_thread{0}, no_dependent_launch{0}, plain_sp{0};
 };
 Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
 thread_local int g_launches = 0;                                      // kernels launched by the last entry-point call
 
-#ifndef LT_PPT32_PACKED
-#define LT_PPT32_PACKED 4          // pixels per thread of the packed fp32 grid kernel (4 or 8)
-#endif
 constexpr int kDefaultChunk64 = 256;   // 32 KB of fp64 records per CTA
 constexpr int kDefaultChunk32 = 1024;  // 64 KB of fp32 records per CTA
 constexpr size_t kAlign = 256;
@@ -190,7 +187,7 @@ int pick_chunk(K kernel, int n_lens, int wanted, size_t rec_bytes, const DeviceI
 
 // pixels per thread: the largest of the candidates that still gives every SM about two tiles
 int pick_ppt(int wanted, int max_ppt, int nx, int ny, const DeviceInfo& d) {
-  if (wanted == 1 || wanted == 2 || wanted == 4 || wanted == 8) return wanted <= max_ppt ? wanted : max_ppt;
+  if (wanted == 1 || wanted == 2 || wanted == 4) return wanted <= max_ppt ? wanted : max_ppt;
   int ppt = max_ppt;
   while (ppt > 1) {
     const long long tiles = (long long)((nx + 32 * ppt - 1) / (32 * ppt)) * ((ny + LT_TILE_H - 1) / LT_TILE_H);
@@ -325,13 +322,8 @@ int launch_f32(const typename Rec64<M>::type* l64, const typename Rec32<M>::type
   // 4 pixels per thread at <= 80 registers (3 CTAs per SM): with a tighter register budget the compiler reloads the
   // constants inside the loop and the kernel, which is bound by issue slots, loses 10 %
   KernelEvents ke(st, hook);
-  return launch_waves(pick_ppt(g_tuning.ppt32, M::kPacked32 ? LT_PPT32_PACKED : 4, a.nx, a.ny, d), a,
+  return launch_waves(pick_ppt(g_tuning.ppt32, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
-                        if constexpr (M::kPacked32 && LT_PPT32_PACKED == 8) {   // four pixel pairs per thread
-                          if (ppt == 8)
-                            return out_wide ? launch_f32_ppt<M, 8, 2, true>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident)
-                                            : launch_f32_ppt<M, 8, 2, false>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
-                        }
                         if (out_wide) {      // mixed mode: the kernel variant that also stores the widened value
                           switch (ppt) {
                             case 1: return launch_f32_ppt<M, 1, 6, true>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
@@ -345,6 +337,49 @@ int launch_f32(const typename Rec64<M>::type* l64, const typename Rec32<M>::type
                           default: return launch_f32_ppt<M, 4, 3, false>(l64, l32, t32, a, out, out_wide, d, st, tiles_x, b, e, resident);
                         }
                       });
+}
+
+// the paper's plain SP version (lt_kernels.cuh): measurement variant selected by lt_set_tuning
+template <class M>
+int launch_f32_plain(const void* d_raw, const typename Rec64<M>::type* l64, const typename Rec32<M>::type* l32,
+                     const LtTables<float>* t32, const GridArgs& a, float2* out, double2* out_wide, const DeviceInfo& d,
+                     cudaStream_t st) {
+  int chunk = 1, grid = 1;
+  const long long n_pix = (long long)a.nx * a.ny;
+  auto go = [&](auto kernel) -> int {
+    int rc = pick_chunk(kernel, a.n_lens, kDefaultChunk32, sizeof(typename Rec32<M>::type), d, chunk);
+    if (rc != LT_OK) return rc;
+    const size_t smem = (size_t)chunk * sizeof(typename Rec32<M>::type);
+    rc = grid_for(kernel, smem, (n_pix + LT_THREADS - 1) / LT_THREADS, d, grid);
+    if (rc != LT_OK) return rc;
+    LT_CUDA(launch_dependent(kernel, grid, LT_THREADS, smem, st, reinterpret_cast<const typename M::Raw*>(d_raw), l64, l32, t32,
+                             a.n_lens, chunk, a.x_min, a.y_min, a.dx, a.nx, a.ny, out, out_wide));
+    ++g_launches;
+    return LT_OK;
+  };
+  return out_wide ? go(lt_grad_f32_plain_kernel<M, true>) : go(lt_grad_f32_plain_kernel<M, false>);
+}
+
+// a9: the fp64 pass of the mixed mode over the quad list (count known on the device only: the grid is sized for the
+// worst case, all quads listed, and CTAs beyond the count leave at once)
+template <class M>
+int launch_quads(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, int quads_per_row,
+                 const unsigned int* list, const LtWsHeader* hdr, const unsigned char* flags, double2* out,
+                 const DeviceInfo& d, cudaStream_t st) {
+  int chunk = 1, grid = 1;
+  const int wanted = g_tuning.chunk64;
+  int rc = pick_chunk(lt_grad_quads_f64_kernel<M>, a.n_lens, wanted > 0 ? wanted : kDefaultChunk64,
+                      sizeof(typename Rec64<M>::type), d, chunk);
+  if (rc != LT_OK) return rc;
+  const size_t smem = (size_t)chunk * sizeof(typename Rec64<M>::type);
+  const long long n_quads = (long long)quads_per_row * a.ny;
+  rc = grid_for(lt_grad_quads_f64_kernel<M>, smem, (n_quads + LT_THREADS - 1) / LT_THREADS, d, grid);
+  if (rc != LT_OK) return rc;
+  KernelEvents ke(st);
+  LT_CUDA(launch_dependent(lt_grad_quads_f64_kernel<M>, grid, LT_THREADS, smem, st, l64, t64, a.n_lens, chunk, a.x_min,
+                           a.y_min, a.dx, a.nx, quads_per_row, list, hdr, flags, out));
+  ++g_launches;
+  return LT_OK;
 }
 
 template <class M, bool FROM_LIST>
@@ -457,7 +492,10 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
     rc = precompute<M>(d_lenses, n_lens, dx, ws, L, st);                                   /* a1 */
     if (rc != LT_OK) return rc;
     if (mode == LT_FP64) return launch_f64<M>(l64, t64, a, (double2*)d_out_grad, dev, st, /*hook=*/false);   /* a2-a7 */
-    if (mode == LT_FP32) return launch_f32<M>(l64, l32, t32, a, (float2*)d_out_grad, dev, st, /*hook=*/false);
+    if (mode == LT_FP32) {
+      if (g_tuning.plain_sp) return launch_f32_plain<M>(d_lenses, l64, l32, t32, a, (float2*)d_out_grad, nullptr, dev, st);
+      return launch_f32<M>(l64, l32, t32, a, (float2*)d_out_grad, dev, st, /*hook=*/false);
+    }
   }
 
   /* LT_MIXED: single precision everywhere, flag, double precision on the flagged pixels */
@@ -476,16 +514,26 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
                              x_min, y_min, dx, nx, ny, md, flags));
     ++g_launches;
   }
-  rc = launch_f32<M>(l64, l32, t32, a, sp, dev, st, /*hook=*/false, (double2*)d_out_grad);
+  rc = g_tuning.plain_sp ? launch_f32_plain<M>(d_lenses, l64, l32, t32, a, sp, (double2*)d_out_grad, dev, st)
+                         : launch_f32<M>(l64, l32, t32, a, sp, dev, st, /*hook=*/false, (double2*)d_out_grad);
   if (rc != LT_OK) return rc;
   {
     long long blocks = (n_pix + LT_FLAG_PPI * 256 - 1) / (LT_FLAG_PPI * 256);
     const long long cap = (long long)dev.sms * 8;
     if (blocks > cap) blocks = cap;
-    LT_CUDA(launch_dependent(lt_flag_kernel, (int)blocks, 256, 0, st, sp, nx, ny, md, flags, list, hdr));   /* a8 */
+    LT_CUDA(launch_dependent(lt_flag_kernel, (int)blocks, 256, 0, st, sp, nx, ny, md, flags, hdr));   /* a8 */
     ++g_launches;
   }
-  return launch_list<M, true>(l64, t64, a, list, hdr, nullptr, 0, n_pix, (double2*)d_out_grad, dev, st);           /* a9 */
+  const int quads_per_row = (nx + 3) / 4;
+  {
+    long long blocks = ((long long)quads_per_row * ny + 255) / 256;
+    const long long cap = (long long)dev.sms * 8;
+    if (blocks > cap) blocks = cap;
+    LT_CUDA(launch_dependent(lt_quad_list_kernel, (int)blocks, 256, 0, st, (const unsigned char*)flags, nx, ny, quads_per_row,
+                             list, hdr));
+    ++g_launches;
+  }
+  return launch_quads<M>(l64, t64, a, quads_per_row, list, hdr, flags, (double2*)d_out_grad, dev, st);        /* a9 */
 }
 
 template <class M>
@@ -616,6 +664,7 @@ int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_s
   g_tuning.staged_host_output = (single_launch >> 1) & 1;
   g_tuning.points_per_thread = (single_launch >> 2) & 1;
   g_tuning.no_dependent_launch = (single_launch >> 3) & 1;
+  g_tuning.plain_sp = (single_launch >> 4) & 1;
   g_tuning.ppt64 = ppt64;
   g_tuning.ppt32 = ppt32;
   g_tuning.chunk64 = chunk64;
@@ -741,7 +790,6 @@ int lt_mixed_rule(const float* d_sp_map, double x_min, double y_min, double dx, 
   const long long cap = (long long)dev.sms * 8;
   if (blocks > cap) blocks = cap;
   lt_flag_kernel<<<(int)blocks, 256, 0, st>>>(reinterpret_cast<const float2*>(d_sp_map), nx, ny, md, d_flags,
-                                              reinterpret_cast<unsigned int*>(ws + L.list),
                                               reinterpret_cast<LtWsHeader*>(ws + L.header));
   LT_CUDA(cudaGetLastError());
   ++g_launches;
@@ -843,7 +891,7 @@ int lt_mixed_last_stats(const void* d_workspace, void* cuda_stream, lt_mixed_sta
   LT_CUDA(cudaMemcpyAsync(&h, d_workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
   LT_CUDA(cudaStreamSynchronize(st));
   out->n_pixels = -1;          /* not recorded in the header: the caller knows nx*ny */
-  out->n_flagged = (long long)h.list_count;
+  out->n_flagged = (long long)h.n_flagged;
   out->n_patch = (long long)h.n_patch;
   out->n_eq25 = (long long)h.n_eq25;
   out->n_eq28 = (long long)h.n_eq28;

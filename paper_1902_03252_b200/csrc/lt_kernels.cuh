@@ -28,10 +28,11 @@
 struct LtWsHeader {                 // first 256 bytes of the workspace; (re)initialised by the precompute kernel
   int bad_blocks;                   // number of slots of the bad-code array written by this call
   int n_lens;
-  unsigned int list_count;          // number of flagged pixels appended to the list (mixed)
+  unsigned int list_count;          // number of quads appended to the recompute list (mixed)
   unsigned int pad0;
   unsigned long long n_patch, n_eq25, n_eq28;
-  unsigned long long pad1[27];
+  unsigned long long n_flagged;     // flagged pixels (patch OR eq. 25 OR eq. 28)
+  unsigned long long pad1[26];
 };
 static_assert(sizeof(LtWsHeader) == 256, "workspace header is 256 bytes");
 
@@ -69,6 +70,7 @@ __global__ void lt_precompute_kernel(const typename M::Raw* __restrict__ raw, in
     hdr->n_patch = 0;
     hdr->n_eq25 = 0;
     hdr->n_eq28 = 0;
+    hdr->n_flagged = 0;
   }
   if (k < n_lens) {
     const typename M::Raw r = raw[k];
@@ -187,13 +189,13 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
   typedef typename M::template Rec<float>::type Rec;
   typedef typename M::template Rec<double>::type Rec64;
   constexpr int TILE_W = 32 * PPT;
-  constexpr bool PACK = M::kPacked32 && !M::kSkyFrame32 && (PPT % 2 == 0);
+  constexpr bool PACK = M::kPacked32 && (PPT % 2 == 0);
   __shared__ typename LtSelect<PACK, LtTables2, LtTables<float>>::type tab;
   Rec* sl = reinterpret_cast<Rec*>(lt_smem);
   lt_grid_dependency_wait();
   // the tables become visible with the first __syncthreads of the chunk loop
   if constexpr (PACK) {
-    lt_stage_tables2(reinterpret_cast<LtTables2*>(&tab), tables);
+    if (M::kTables) lt_stage_tables2(reinterpret_cast<LtTables2*>(&tab), tables);
   } else if (M::kTables) {
     lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
   }
@@ -239,7 +241,13 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
 #pragma unroll 1
       for (int k = 0; k < cnt; ++k) {
         const Rec L = sl[k];
-        if constexpr (M::kSkyFrame32) {
+        if constexpr (M::kSkyFrame32 && PACK) {       // two pixels of the thread per instruction (lt_math.cuh)
+          const float d2 = fmaf(jl, fdx, L.y0);
+          const auto row = M::template row<float>(d2, L);
+#pragma unroll
+          for (int p = 0; p < PPT; p += 2)
+            M::interact_sky_x2(lt2_fma(lt2(il[p], il[p + 1]), lt2(fdx), lt2(L.x0)), row, L, tab, H1[p / 2], H2[p / 2]);
+        } else if constexpr (M::kSkyFrame32) {
           const float d2 = fmaf(jl, fdx, L.y0);
           const auto row = M::template row<float>(d2, L);
 #pragma unroll
@@ -284,6 +292,58 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
           if (WIDE) out_wide[(size_t)j * nx + i] = make_double2((double)G1[p], (double)G2[p]);
         }
       }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ fp32, plain coordinates
+// The paper's own SP version: "identical [to the DP version] up to the change in precision", i.e. Algorithm 1
+// with theta, theta_center and their difference (l.3-4) all in fp32 -- no tile centre formed in fp64.  Not the product's
+// fp32 mode: it exists so that the error that the tile-centre scheme removes can be measured (the |theta_c| / |dtheta|
+// term of (A.65), the reason for the paper's DP patches around the lens centres; Fig. 9).
+// Selected by lt_set_tuning (single_launch bit 4).  One pixel per thread, scalar arithmetic, no claim on speed.
+template <class M, bool WIDE>
+__global__ void __launch_bounds__(LT_THREADS)
+lt_grad_f32_plain_kernel(const typename M::Raw* __restrict__ raw, const typename M::template Rec<double>::type* __restrict__ lens64,
+                         const typename M::template Rec<float>::type* __restrict__ lens32,
+                         const LtTables<float>* __restrict__ tables, int n_lens, int chunk, double x_min, double y_min,
+                         double dx, int nx, int ny, float2* __restrict__ out, double2* __restrict__ out_wide) {
+  extern __shared__ __align__(16) unsigned char lt_smem[];
+  typedef typename M::template Rec<float>::type Rec;
+  __shared__ LtTables<float> tab;
+  Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  lt_grid_dependency_wait();
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  const float fx = (float)x_min, fy = (float)y_min, fdx = (float)dx;
+  const size_t n_pix = (size_t)nx * ny;
+  for (size_t base = (size_t)blockIdx.x * LT_THREADS; base < n_pix; base += (size_t)gridDim.x * LT_THREADS) {
+    const size_t p = base + threadIdx.x;
+    const size_t q = p < n_pix ? p : n_pix - 1;
+    const int j = (int)(q / (size_t)nx), i = (int)(q - (size_t)j * nx);
+    const float t1 = __fadd_rn(fx, __fmul_rn((float)i, fdx));      // a2 in fp32
+    const float t2 = __fadd_rn(fy, __fmul_rn((float)j, fdx));
+    float G1 = 0.f, G2 = 0.f;
+    for (int b0 = 0; b0 < n_lens; b0 += chunk) {
+      const int cnt = min(chunk, n_lens - b0);
+      __syncthreads();
+      for (int k = threadIdx.x; k < cnt; k += LT_THREADS) {
+        Rec F = lens32[b0 + k];
+        M::unscale32(lens64[b0 + k], F);                           // the rotation constants without the pixel size
+        F.x0 = (float)raw[b0 + k].x;                               // theta_center rounded to fp32
+        F.y0 = (float)raw[b0 + k].y;
+        sl[k] = F;
+      }
+      __syncthreads();
+#pragma unroll 1
+      for (int k = 0; k < cnt; ++k) {
+        const Rec L = sl[k];
+        const float d2 = __fsub_rn(t2, L.y0);                      // Alg. 1 l.4 in fp32
+        M::template interact_sky<float>(__fsub_rn(t1, L.x0), M::template row<float>(d2, L), L, tab, G1, G2);   // l.3, l.5-14
+      }
+    }
+    if (p < n_pix) {
+      out[p] = make_float2(G1, G2);
+      if (WIDE) out_wide[p] = make_double2((double)G1, (double)G2);
     }
   }
 }
@@ -381,6 +441,71 @@ lt_grad_list_f64_kernel(const typename M::template Rec<double>::type* __restrict
   for (long long g = blockIdx.x; g < n_rest; g += gridDim.x)
     lt_list_group<M, FROM_LIST, 1>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
                                 rest0 + g * LT_THREADS, total, out);
+}
+
+// ------------------------------------------------------------------------------------------------ fp64 quad kernel (a9)
+// The fp64 pass of the mixed mode.  Work list: the quads of lt_quad_list_kernel (lt_mixed.cuh), count read from the
+// workspace header on the device (no host round trip).  A thread owns one quad = four neighbouring pixels of a row, so
+// its lens loop is the grid kernel's: one row term per lens shared by four interact_abs calls, same operations in the
+// same order -- identical bits for identical pixels at the grid kernel's instruction count (the per-pixel list kernel
+// below forms the row terms once per pixel).  All four pixels are recomputed, the flagged ones are stored.
+template <class M>
+__global__ void __launch_bounds__(LT_THREADS, 2)
+lt_grad_quads_f64_kernel(const typename M::template Rec<double>::type* __restrict__ lens,
+                         const LtTables<double>* __restrict__ tables, int n_lens, int chunk, double x_min, double y_min,
+                         double dx, int nx, int quads_per_row, const unsigned int* __restrict__ list,
+                         const LtWsHeader* __restrict__ hdr, const unsigned char* __restrict__ flags,
+                         double2* __restrict__ out) {
+  extern __shared__ __align__(16) unsigned char lt_smem[];
+  typedef typename M::template Rec<double>::type Rec;
+  __shared__ LtTables<double> tab;
+  Rec* sl = reinterpret_cast<Rec*>(lt_smem);
+  lt_grid_dependency_wait();
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  __syncthreads();
+  const long long total = (long long)hdr->list_count;
+  const bool single = n_lens <= chunk;
+  if (single) {
+    lt_copy16(sl, lens, n_lens * (int)(sizeof(Rec) / 16));
+    __syncthreads();
+  }
+  // whole CTAs iterate together (the lens chunks are staged cooperatively)
+  for (long long first = (long long)blockIdx.x * LT_THREADS; first < total; first += (long long)gridDim.x * LT_THREADS) {
+    const long long g = first + threadIdx.x;
+    const bool live = g < total;
+    const unsigned int q = live ? list[g] : 0u;
+    const int j = (int)(q / (unsigned int)quads_per_row);
+    const int i0 = (int)(q - (unsigned int)j * (unsigned int)quads_per_row) * 4;
+    const size_t p0 = (size_t)j * nx + (size_t)i0;
+    const double t2 = __dadd_rn(y_min, __dmul_rn((double)j, dx));
+    double t1[4], G1[4], G2[4];
+    bool keep[4];
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      t1[p] = __dadd_rn(x_min, __dmul_rn((double)(i0 + p), dx));
+      G1[p] = 0.0;
+      G2[p] = 0.0;
+      keep[p] = live && i0 + p < nx && flags[p0 + p] != 0;
+    }
+    for (int base = 0; base < n_lens; base += chunk) {
+      const int cnt = min(chunk, n_lens - base);
+      if (!single) {
+        __syncthreads();
+        lt_copy16(sl, lens + base, cnt * (int)(sizeof(Rec) / 16));
+        __syncthreads();
+      }
+#pragma unroll 1
+      for (int k = 0; k < cnt; ++k) {
+        const Rec L = sl[k];
+        const auto row = M::template row_abs<double>(t2, L);
+#pragma unroll
+        for (int p = 0; p < 4; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
+      }
+    }
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+      if (keep[p]) out[p0 + p] = make_double2(G1[p], G2[p]);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ short point lists

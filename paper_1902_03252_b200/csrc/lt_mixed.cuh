@@ -59,14 +59,15 @@ __global__ void lt_patch_kernel(const typename M::Raw* __restrict__ raw, int n_l
   }
 }
 
-// a8, part 2: criteria on the fp32 map, merge with the patch bit (the fp32 kernel has already written the widened fp32
-// values into the fp64 output, R17),
-// append flagged pixels to the compact list (CTA-aggregated atomic; the order of the list is irrelevant because
-// every pixel is recomputed independently), count.
+// a8, part 2: criteria on the fp32 map, merged with the patch bit (the fp32 kernel has already written the widened fp32
+// values into the fp64 output, R17), flag byte written back, counts.
 // A CTA takes LT_FLAG_PPI * 256 consecutive pixels per iteration, LT_FLAG_PPI per thread (256 apart, so every load is
-// coalesced): the loads of the four pixels and their neighbours are in flight together and the two barriers and the
-// atomic of the append are paid once per 1024 pixels (one pixel per thread: 19 % of the HBM rate at 45 M pixels, bound
-// by load latency and barriers; profiles/r01f_flag_kernel.md).
+// coalesced): the loads of the four pixels and their neighbours are in flight together.
+// a8, part 3 (lt_quad_list_kernel): the flagged pixels are handed to the fp64 pass as a compact list of QUADS -- four
+// neighbouring pixels of one row, i = 4 iq .. 4 iq + 3, listed when any of them is flagged.  The fp64 pass recomputes all
+// four (they share the row terms of every lens exactly as the four pixels of a thread do in the grid kernel) and
+// stores the flagged ones only.  Flagged pixels come in runs (patches are boxes, the critical-line bands are many pixels
+// wide): on the SIE benchmark the listed quads hold 1.005 x the flagged pixels.
 #define LT_FLAG_PPI 4
 struct LtFlagLoads { float2 a, bx, by; unsigned char f0; bool fwd_x, fwd_y; };
 // the loads of one pixel, branch-free so that those of the LT_FLAG_PPI pixels of a thread are issued back to back:
@@ -107,18 +108,13 @@ __device__ __forceinline__ unsigned char lt_flag_decide(const LtFlagLoads& v, in
 
 __global__ void __launch_bounds__(256)
 lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, unsigned char* __restrict__ flags,
-               unsigned int* __restrict__ list, LtWsHeader* __restrict__ hdr) {
+               LtWsHeader* __restrict__ hdr) {
   lt_grid_dependency_wait();
   const size_t n_pix = (size_t)nx * ny;
   constexpr size_t TILE = (size_t)LT_FLAG_PPI * 256;
   const unsigned lane = threadIdx.x & 31;
-  const unsigned wrp = threadIdx.x >> 5;
-  unsigned long long c_patch = 0, c25 = 0, c28 = 0;
-  // whole CTAs iterate together so that the ballots see a full mask and the barriers are reached by every thread
-  __shared__ unsigned int seg_base[LT_FLAG_PPI * 8];          // segment s = k * 8 + warp: 32 pixels of sub-tile k
+  unsigned long long c_any = 0, c_patch = 0, c25 = 0, c28 = 0;
   for (size_t base = (size_t)blockIdx.x * TILE; base < n_pix; base += (size_t)gridDim.x * TILE) {
-    unsigned char f[LT_FLAG_PPI];
-    unsigned m[LT_FLAG_PPI];
     LtFlagLoads v[LT_FLAG_PPI];
 #pragma unroll
     for (int k = 0; k < LT_FLAG_PPI; ++k) {
@@ -128,52 +124,62 @@ lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, uns
 #pragma unroll
     for (int k = 0; k < LT_FLAG_PPI; ++k) {
       const size_t p = base + (size_t)k * 256 + threadIdx.x;
-      f[k] = 0;
       if (p < n_pix) {
-        f[k] = lt_flag_decide(v[k], nx, ny, mp);
-        flags[p] = f[k];
-        c_patch += f[k] & 1;
-        c25 += (f[k] >> 1) & 1;
-        c28 += (f[k] >> 2) & 1;
+        const unsigned char f = lt_flag_decide(v[k], nx, ny, mp);
+        flags[p] = f;
+        c_any += f != 0;
+        c_patch += f & 1;
+        c25 += (f >> 1) & 1;
+        c28 += (f >> 2) & 1;
       }
     }
-#pragma unroll
-    for (int k = 0; k < LT_FLAG_PPI; ++k) {
-      m[k] = __ballot_sync(0xffffffffu, f[k] != 0);
-      if (lane == 0) seg_base[k * 8 + wrp] = (unsigned int)__popc(m[k]);
-    }
-    __syncthreads();
-    // append: one atomic per CTA and iteration; warp 0 scans the LT_FLAG_PPI * 8 = 32 segment counts
-    if (wrp == 0) {
-      static_assert(LT_FLAG_PPI * 8 == 32, "one segment per lane of warp 0");
-      const unsigned int cnt = seg_base[lane];
-      unsigned int incl = cnt;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
-        if ((int)lane >= o) incl += v;
-      }
-      unsigned int cta_base = 0;
-      if (lane == 31 && incl) cta_base = atomicAdd(&hdr->list_count, incl);
-      cta_base = __shfl_sync(0xffffffffu, cta_base, 31);
-      seg_base[lane] = cta_base + incl - cnt;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int k = 0; k < LT_FLAG_PPI; ++k)
-      if (f[k] != 0)
-        list[seg_base[k * 8 + wrp] + __popc(m[k] & ((1u << lane) - 1u))] = (unsigned int)(base + (size_t)k * 256 + threadIdx.x);
-    __syncthreads();                                          // seg_base is rewritten by the next iteration
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
+    c_any += __shfl_xor_sync(0xffffffffu, c_any, o);
     c_patch += __shfl_xor_sync(0xffffffffu, c_patch, o);
     c25 += __shfl_xor_sync(0xffffffffu, c25, o);
     c28 += __shfl_xor_sync(0xffffffffu, c28, o);
   }
   if (lane == 0) {
+    if (c_any) atomicAdd(&hdr->n_flagged, c_any);
     if (c_patch) atomicAdd(&hdr->n_patch, c_patch);
     if (c25) atomicAdd(&hdr->n_eq25, c25);
     if (c28) atomicAdd(&hdr->n_eq28, c28);
+  }
+}
+
+// a8, part 3: compact list of the quads (j, iq) -> j * quads_per_row + iq that hold a flagged pixel.  One quad per thread,
+// warp-aggregated append (one atomic per warp and iteration); the order of the list is irrelevant because every quad is
+// recomputed independently.  Flag bytes are read with one 32-bit load where the quad is 4-byte aligned and inside the row.
+__global__ void __launch_bounds__(256)
+lt_quad_list_kernel(const unsigned char* __restrict__ flags, int nx, int ny, int quads_per_row,
+                    unsigned int* __restrict__ list, LtWsHeader* __restrict__ hdr) {
+  lt_grid_dependency_wait();
+  const unsigned lane = threadIdx.x & 31;
+  const size_t n_quads = (size_t)quads_per_row * ny;
+  // whole warps iterate together so that the ballots see a full mask
+  for (size_t base = ((size_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u)); base < n_quads;
+       base += (size_t)gridDim.x * blockDim.x) {
+    const size_t q = base + lane;
+    bool any = false;
+    if (q < n_quads) {
+      const size_t j = q / (size_t)quads_per_row;
+      const int i0 = (int)(q - j * (size_t)quads_per_row) * 4;
+      const size_t p = j * (size_t)nx + (size_t)i0;
+      if (i0 + 3 < nx && (p & 3) == 0) {
+        any = *reinterpret_cast<const unsigned int*>(flags + p) != 0u;
+      } else {
+        for (int k = 0; k < 4; ++k)
+          if (i0 + k < nx) any = any || flags[p + k] != 0;
+      }
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, any);
+    if (m) {
+      unsigned int warp_base = 0;
+      if (lane == 0) warp_base = atomicAdd(&hdr->list_count, (unsigned int)__popc(m));
+      warp_base = __shfl_sync(0xffffffffu, warp_base, 0);
+      if (any) list[warp_base + __popc(m & ((1u << lane) - 1u))] = (unsigned int)q;
+    }
   }
 }

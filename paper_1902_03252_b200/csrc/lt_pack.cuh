@@ -169,6 +169,10 @@ struct LtDpieModel {
   static LT_HD void poison(LtLens<double>& L) { lt_poison_lens(L); }
   static LT_HD void round(const LtLens<double>& D, double dx, LtLens<float>& F) { lt_round_lens(D, dx, F); }
   static LT_HD double patch_scale(const Raw& r) { return r.b0; }
+  // fp32 record for the plain-coordinate kernel: rotation constants per arcsec instead of per pixel
+  static LT_HD void unscale32(const LtLens<double>& D, LtLens<float>& F) {
+    F.cx = (float)D.cx; F.sx = (float)D.sx; F.cy = (float)D.cy; F.sy = (float)D.sy;
+  }
   template <class T> static LT_HD Row<T> row(const T d2, const LtLens<T>& L) { return Row<T>{d2 * L.sx, d2 * L.cy}; }
   // GRID = called from the fp64 grid kernel (lt_sqrt_h: where a hoisted constant pays)
   template <class T, bool GRID = false>
@@ -198,12 +202,19 @@ struct LtSieModel {
   template <class T> struct Rec { typedef LtSieLens<T> type; };
   static constexpr bool kTables = false;
   static constexpr bool kSkyFrame32 = true;
-  static constexpr bool kPacked32 = false;
+  static constexpr bool kPacked32 = true;
+#if defined(__CUDACC__)
+  static __device__ __forceinline__ void interact_sky_x2(const lt_f2 d1, const LtSieRow<float>& r, const LtSieLens<float>& L,
+                                                         const LtTables2&, lt_f2& G1, lt_f2& G2) {
+    lt_sie_interact_x2(d1, r, L, G1, G2);
+  }
+#endif
   static LT_HD bool valid(const Raw& r) { return lt_sie_valid(r); }
   static LT_HD void pack(const Raw& r, LtSieLens<double>& L) { lt_pack_sie(r, L); }
   static LT_HD void poison(LtSieLens<double>& L) { lt_poison_sie(L); }
   static LT_HD void round(const LtSieLens<double>& D, double dx, LtSieLens<float>& F) { lt_round_sie(D, dx, F); }
   static LT_HD double patch_scale(const Raw& r) { return r.b0; }
+  static LT_HD void unscale32(const LtSieLens<double>&, LtSieLens<float>&) {}
   template <class T> static LT_HD LtSieRow<T> row(const T d2, const LtSieLens<T>& L) { return lt_sie_row<T>(d2, L); }
   template <class T>
   static LT_HD void interact_lens(const T, const T, const LtSieLens<T>&, const LtTables<T>&, T&, T&) {}   // unused
@@ -230,6 +241,7 @@ struct LtNfwModel {
   static LT_HD void poison(LtNfwLens<double>& L) { lt_poison_nfw(L); }
   static LT_HD void round(const LtNfwLens<double>& D, double dx, LtNfwLens<float>& F) { lt_round_nfw(D, dx, F); }
   static LT_HD double patch_scale(const Raw& r) { return 4.0 * r.ks * r.rs; }
+  static LT_HD void unscale32(const LtNfwLens<double>&, LtNfwLens<float>&) {}
   template <class T> static LT_HD LtSieRow<T> row(const T d2, const LtNfwLens<T>& L) {
     return LtSieRow<T>{d2, L.q12 * d2, L.q22 * d2};
   }

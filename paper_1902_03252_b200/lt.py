@@ -471,12 +471,18 @@ def lt_rule_audit(sp_map, dp_map, x_min, y_min, dx, centres=None, flags=None, wa
                                ctypes.c_void_p(flags.data_ptr() if flags is not None else None),
                                ctypes.c_void_p(viol.data_ptr() if viol is not None else None),
                                ctypes.c_void_p(d_res.data_ptr()), _stream(stream)), "lt_rule_audit")
+    _keep(stream, centres, d_res, viol)
+    return d_res, viol
+
+
+def lt_rule_audit_result(d_result, dx, stream=None):
+    """(synchronises) the fields of the lt_audit_result that lt_rule_audit left in device memory, as a dict"""
     h = lt_audit_result()
-    _check(lib().lt_rule_audit_result(ctypes.c_void_p(d_res.data_ptr()), float(dx), _stream(stream), ctypes.byref(h)),
+    _check(lib().lt_rule_audit_result(ctypes.c_void_p(d_result.data_ptr()), float(dx), _stream(stream), ctypes.byref(h)),
            "lt_rule_audit_result")
     out = {name: getattr(h, name) for name, _ in lt_audit_result._fields_ if name != "max_err_by_distance"}
     out["max_err_by_distance"] = list(h.max_err_by_distance)
-    return out, viol
+    return out
 
 
 def lt_peak_probe(which, iters=1 << 16, stream=None):

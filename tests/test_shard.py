@@ -43,6 +43,48 @@ def _coords_map(lenses, x_min, y_min, dx, nx, ny, mode):
     return torch.stack([x_min + i * dx, y_min + j * dx], dim=-1)
 
 
+def _stencil_map(lenses, x_min, y_min, dx, nx, ny, mode):
+    """CPU stand-in for lt_gradient_grid with the data dependence of the mixed mode (eq. 24 / 27): in mode 2
+    a pixel's value also depends on its LOWER neighbour's, and the first row of a call uses the forward neighbour (R12).
+    Values are exact integers derived from the GLOBAL pixel indices (recovered from the coordinates), so the sharded and
+    the unsharded maps can be compared bit for bit."""
+    import torch
+    jg = torch.round((y_min + torch.arange(ny, dtype=torch.float64) * dx - 5.0) / dx)           # global row index
+    ig = torch.arange(nx, dtype=torch.float64)
+    base = torch.stack([(jg[:, None] * 131.0 + ig[None, :] * 7.0) % 1009.0,
+                        (jg[:, None] * 17.0 + ig[None, :] * 313.0) % 997.0], dim=-1)
+    if mode != 2 or ny < 2:
+        return base
+    out = base.clone()
+    out[1:] += 0.5 * base[:-1]
+    out[0] += 0.5 * base[1]
+    return out
+
+
+def _worker_stencil(rank, world, port, ny, nx, ret):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        x_min, y_min, dx = -3.0, 5.0, 0.5
+        ok = True
+        for mode in (0, 2):
+            b, out = shard.compute_block(_stencil_map, None, x_min, y_min, dx, nx, ny, mode, rank, world)
+            assert b.halo == (1 if (mode == 2 and rank > 0) else 0)
+            full = shard.all_gather_rows(out, ny, nx, rank, world)
+            ref = _stencil_map(None, x_min, y_min, dx, nx, ny, mode)
+            ok = ok and bool(torch.equal(full, ref))
+            if mode == 2 and rank > 0:
+                # without the halo row the block's first row would have used its forward neighbour: a different map
+                wrong = _stencil_map(None, x_min, y_min + b.j0 * dx, dx, nx, b.j1 - b.j0, mode)
+                ok = ok and not bool(torch.equal(wrong, ref[b.j0:b.j1]))
+        ret[rank] = ok
+    finally:
+        dist.destroy_process_group()
+
+
 def _worker(rank, world, port, ny, nx, mode, ret):
     import torch
     import torch.distributed as dist
@@ -82,6 +124,18 @@ def test_gather_world_size_2_gloo(ny, mode):
     with mp.Manager() as m:
         ret = m.dict()
         mp.spawn(_worker, args=(world, _free_port(), ny, 5, mode, ret), nprocs=world, join=True)
+        assert dict(ret) == {0: True, 1: True}
+
+
+@pytest.mark.parametrize("ny", [9, 16])
+def test_mixed_halo_through_the_gather_world_size_2_gloo(ny):
+    """compute_block with a map function that has the mixed mode's neighbour dependence, the blocks gathered over gloo:
+    bit-equal to the unsharded map in both modes; the self-computed halo row is what makes it so."""
+    import torch.multiprocessing as mp
+    world = 2
+    with mp.Manager() as m:
+        ret = m.dict()
+        mp.spawn(_worker_stencil, args=(world, _free_port(), ny, 6, ret), nprocs=world, join=True)
         assert dict(ret) == {0: True, 1: True}
 
 
