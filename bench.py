@@ -66,7 +66,7 @@ KERNEL_NAME = {"fp64": "lt_grad_f64_kernel", "fp32": "lt_grad_f32_kernel", "mixe
 # holds the SMSP's pipe for one warp).  fp64 / mixed: FP64 instructions, 16 lanes, 2 cycles; fp32: the FMA pipe takes a
 # packed FFMA2 / FMUL2 / FADD2 for 2 cycles (32 lanes, two results each); SIE fp32: one MUFU.RSQ per interaction on the
 # 4-lane XU, 8 cycles -- above its 7.75 FMA-pipe cycles.
-PIPE_FLOOR = {("dpie", "fp64"): ("fp64", 60.5, 2.0), ("dpie", "mixed"): ("fp64", 60.5, 2.0),
+PIPE_FLOOR = {("dpie", "fp64"): ("fp64", 61.75, 2.0), ("dpie", "mixed"): ("fp64", 61.75, 2.0),
               ("dpie", "fp32"): ("fp32 fma (packed pairs)", 20.25, 2.0),
               ("sie", "fp64"): ("fp64", 12.75, 2.0), ("sie", "mixed"): ("fp64", 12.75, 2.0),
               ("sie", "fp32"): ("xu (MUFU.RSQ)", 1.0, 8.0)}

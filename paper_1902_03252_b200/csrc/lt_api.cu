@@ -812,15 +812,16 @@ int lt_find_images(const double* d_grad, double x_min, double y_min, double dx, 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   LT_CUDA(cudaMemsetAsync(d_n_hits, 0, sizeof(int), st));
   if (n_sources == 0) return LT_OK;
-  const int tiles_x = (nx - 1 + 31) / 32, tiles_y = (ny - 1 + 7) / 8;
-  const long long n_tiles = (long long)tiles_x * tiles_y;
-  long long grid = (long long)dev.sms * 8;
-  if (grid > n_tiles) grid = n_tiles;
+  const int n_strips = (nx - 1 + LT_FI_STRIP - 1) / LT_FI_STRIP, n_row_blocks = (ny - 1 + LT_FI_BLOCK_ROWS - 1) / LT_FI_BLOCK_ROWS;
+  const long long n_items = (long long)n_strips * n_row_blocks;            // one warp each
+  int grid = 1;
+  const int rc2 = grid_for(lt_find_images_kernel, 0, (n_items + 7) / 8, dev, grid, 256);
+  if (rc2 != LT_OK) return rc2;
   KernelEvents ke(st);
-  lt_find_images_kernel<<<(int)grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_grad), x_min, y_min, dx, nx, ny,
-                                                   dls_dos, reinterpret_cast<const double2*>(d_sources), n_sources,
-                                                   tiles_x, (int)n_tiles, reinterpret_cast<LtImageHit*>(d_hits), max_hits,
-                                                   d_n_hits);
+  lt_find_images_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_grad), x_min, y_min, dx, nx, ny,
+                                              dls_dos, reinterpret_cast<const double2*>(d_sources), n_sources,
+                                              n_strips, (int)n_items, reinterpret_cast<LtImageHit*>(d_hits), max_hits,
+                                              d_n_hits);
   LT_CUDA(cudaGetLastError());
   ++g_launches;
   return LT_OK;

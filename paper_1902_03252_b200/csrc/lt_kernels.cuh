@@ -232,8 +232,9 @@ lt_grad_f32_kernel(const typename M::template Rec<double>::type* __restrict__ le
           F.x0 = (float)(cx - D.x0);
           F.y0 = (float)(cy - D.y0);
         } else {                                    // (scaled) lens-frame position of the tile centre
-          F.x0 = (float)fma(cx, D.cx, fma(cy, D.sx, -D.x0));
-          F.y0 = (float)fma(-cx, D.sy, fma(cy, D.cy, -D.y0));
+          const double d1 = cx - D.x0, d2 = cy - D.y0;
+          F.x0 = (float)fma(d1, D.cx, d2 * D.sx);
+          F.y0 = (float)fma(-d1, D.sy, d2 * D.cy);
         }
         sl[k] = F;
       }

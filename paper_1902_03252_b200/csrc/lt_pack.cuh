@@ -17,10 +17,11 @@ LT_HD bool lt_lens_valid(const LtRawLens& r) {
   return fin && r.e >= 0.0 && r.e < 1.0 && r.rcore > 0.0 && r.rcut > r.rcore;
 }
 
-// fp64 record.  The translation of Alg. 1 l.3-4 is folded into the rotation of l.5-6: X = cx (t1 - xc) + sx (t2 - yc) =
-// cx t1 + sx t2 - X0 with X0 = cx xc + sx yc formed once per lens (two FMAs per coordinate and pixel instead of a
-// subtraction and an FMA; the rounding of X0, 1e-16 of |theta_c|, is to the lens-frame coordinate what the rounding of
-// the pixel coordinate itself is).
+// fp64 record.  x0, y0 = lens centre.  (Folding the translation of Alg. 1 l.3-4 into the rotation, X = cx t1 + sx t2 - X0
+// with X0 = cx xc + sx yc formed once per lens, saves 1.25 FP64 instructions per interaction and 0.8 % of the fp64 time,
+// but X0 carries a rounding of 1e-16 |theta_c|: next to a steep centre -- rcore = 1e-4", central slope b0 / (2 rcore) =
+// 5e4 -- that alone is 1.5e-11 of max|alpha| (tests/test_gpu_parity.py: test_fp64_kernel_beyond_the_configs).  Measured,
+// not kept: the difference theta - theta_center is formed first, exactly as Alg. 1 states it.)
 LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
   double s, c;
   sincos(r.phi, &s, &c);
@@ -36,9 +37,8 @@ LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
   L.sx = qf * s;
   L.cy = rf * c;
   L.sy = rf * s;
-  // scaled lens-frame coordinates of the sky origin, negated: X = cx t1 + sx t2 - X0, Y = cy t2 - sy t1 - Y0
-  L.x0 = fma(L.cx, r.x, L.sx * r.y);
-  L.y0 = fma(L.cy, r.y, -(L.sy * r.x));
+  L.x0 = r.x;
+  L.y0 = r.y;
   L.Kc = (ome * r.rcore * rf) * (ome * r.rcore * rf);  // q^2 s_c^2 / f^2
   L.Kt = (ome * r.rcut * rf) * (ome * r.rcut * rf);
   L.sc = sc * rf;
@@ -189,12 +189,10 @@ struct LtDpieModel {
     interact_lens<T, GRID>(X, Y, L, tab, G1, G2);
   }
   // the same from the absolute sky coordinates (t1, t2) of the pixel: what the fp64 kernels call
-  template <class T> static LT_HD Row<T> row_abs(const T t2, const LtLens<T>& L) {
-    return Row<T>{lt_fma(t2, L.sx, -L.x0), lt_fma(t2, L.cy, -L.y0)};
-  }
+  template <class T> static LT_HD Row<T> row_abs(const T t2, const LtLens<T>& L) { return row<T>(t2 - L.y0, L); }   // l.4
   template <class T, bool GRID = false>
   static LT_HD void interact_abs(const T t1, const Row<T>& r, const LtLens<T>& L, const LtTables<T>& tab, T& G1, T& G2) {
-    interact_sky<T, GRID>(t1, r, L, tab, G1, G2);
+    interact_sky<T, GRID>(t1 - L.x0, r, L, tab, G1, G2);                                                           // l.3
   }
 };
 struct LtSieModel {

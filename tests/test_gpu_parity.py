@@ -339,9 +339,12 @@ def test_calibration_tool_on_small_workloads(env):
         assert tc["calibrated_rule"]["violating_and_missed"] == 0
         assert tc["calibrated_rule"]["flagged_fraction"] <= tc["criterion"]["flagged_fraction"] + 1e-12
         assert tc["implied_m_max_no_patches"] > 3.26
-        assert pl["sp_error_arcsec"]["max"] > tc["sp_error_arcsec"]["max"]
-        near = list(pl["max_sp_error_by_distance_px"].values())
-        assert max(near[:3]) >= max(near[5:])                  # plain SP: worst within a few pixels of a centre
+        assert pl["sp_error_arcsec"]["max"] >= tc["sp_error_arcsec"]["max"]
+        if model == "sie":                                     # the paper's own case: SIS direction theta / R at the centres
+            near = list(pl["max_sp_error_by_distance_px"].values())
+            assert max(near[:3]) > 3 * max(near[5:])           # plain SP: worst within a few pixels of a centre
+            flat = list(tc["max_sp_error_by_distance_px"].values())
+            assert max(flat[:3]) < 3 * max(flat[5:])           # tile-centre coordinates: no growth towards the centres
         print(W.name, "plain", pl["sp_error_arcsec"], pl["max_sp_error_by_distance_px"])
         print(W.name, "tile centre", tc["sp_error_arcsec"], tc["max_sp_error_by_distance_px"])
 
