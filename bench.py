@@ -752,6 +752,7 @@ def run_ours(args, W):
                 consumers(B, W, r, line)
             p64, p32 = lt.lt_peak_probe(0, 1 << 15), lt.lt_peak_probe(1, 1 << 16)
             line["peak_probe"] = {"fp64_tflops": p64 / 1e12, "fp32_tflops": p32 / 1e12,
+                                  "fp32_packed_ffma2_tflops": lt.lt_peak_probe(2, 1 << 15) / 1e12,
                                   "how": "dependent-free FMA chains, full grid, same process"}
             line["roofline"]["frac_of_probe"] = line["roofline"]["achieved"] / (
                 (p64 if LANES[args.mode] == 64 else p32) / 1e12)

@@ -342,7 +342,9 @@ int lt_rule_audit_result(const lt_audit_result* d_result, double dx, void* cuda_
 
 /* FMA-chain microbenchmarks used by bench.py to confirm the FP64 / FP32 peaks on the device in the same run
  * (SURVEY 8(d)): runs `iters` dependent-free FMAs per thread on a full grid; returns achieved FLOP/s in *flops_out
- * (2 flops per FMA).  Synchronises.  which: 0 = fp64, 1 = fp32. */
+ * (2 flops per FMA).  Synchronises.  which: 0 = fp64, 1 = fp32, 2 = fp32 in packed pairs (FFMA2: two FMAs per
+ * instruction -- the same FLOP/s as which = 1 where the FP32 pipe takes a packed instruction for two cycles, which is
+ * what this chip does: packing saves issue slots, not pipe cycles). */
 int lt_peak_probe(int which, int iters, double* flops_out, void* cuda_stream);
 
 #ifdef __cplusplus

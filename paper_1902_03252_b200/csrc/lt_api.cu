@@ -448,6 +448,22 @@ __global__ void __launch_bounds__(256) lt_probe_kernel(int iters, T seed) {
   }
 }
 
+// the same with packed pairs (FFMA2): two results per instruction; which = 2 of lt_peak_probe
+__global__ void __launch_bounds__(256) lt_probe_kernel_x2(int iters, float seed) {
+  float2 a[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) a[i] = make_float2(seed + (float)threadIdx.x + (float)i, seed - (float)i);
+  const float2 m = make_float2(0.999999f, 0.999999f), c = make_float2(1e-6f, 1e-6f);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = __ffma2_rn(a[i], m, c);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += a[i].x + a[i].y;
+  if (s == -12345.678f) lt_probe_sink32 = s;
+}
+
 // ------------------------------------------------------------------------------------------------ entry points, per lens model
 namespace {
 
@@ -958,7 +974,7 @@ int lt_rule_audit_result(const lt_audit_result* d_result, double dx, void* cuda_
 
 int lt_peak_probe(int which, int iters, double* flops_out, void* cuda_stream) {
   if (!flops_out) return LT_ERR_NULL_POINTER;
-  if ((which != 0 && which != 1) || iters < 1) return LT_ERR_BAD_SIZE;
+  if (which < 0 || which > 2 || iters < 1) return LT_ERR_BAD_SIZE;
   DeviceInfo dev;
   const int rc = device_info(dev);
   if (rc != LT_OK) return rc;
@@ -970,7 +986,8 @@ int lt_peak_probe(int which, int iters, double* flops_out, void* cuda_stream) {
   for (int rep = 0; rep < 2; ++rep) {      /* first pass warms up */
     LT_CUDA(cudaEventRecord(e0, st));
     if (which == 0) lt_probe_kernel<double><<<grid, 256, 0, st>>>(iters, 1.0);
-    else lt_probe_kernel<float><<<grid, 256, 0, st>>>(iters, 1.0f);
+    else if (which == 1) lt_probe_kernel<float><<<grid, 256, 0, st>>>(iters, 1.0f);
+    else lt_probe_kernel_x2<<<grid, 256, 0, st>>>(iters, 1.0f);
     LT_CUDA(cudaGetLastError());
     LT_CUDA(cudaEventRecord(e1, st));
     LT_CUDA(cudaEventSynchronize(e1));
@@ -979,7 +996,7 @@ int lt_peak_probe(int which, int iters, double* flops_out, void* cuda_stream) {
   LT_CUDA(cudaEventElapsedTime(&ms, e0, e1));
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
-  *flops_out = 2.0 * 8.0 * (double)iters * 256.0 * (double)grid / ((double)ms * 1e-3);
+  *flops_out = (which == 2 ? 2.0 : 1.0) * 2.0 * 8.0 * (double)iters * 256.0 * (double)grid / ((double)ms * 1e-3);
   return LT_OK;
 }
 
