@@ -114,6 +114,10 @@ class ClockSampler:
             nv.nvmlInit()
             self.nv, self.h = nv, nv.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+            try:
+                self.tdp_w = nv.nvmlDeviceGetPowerManagementLimit(self.h) / 1000.0
+            except Exception:  # noqa: BLE001
+                self.tdp_w = None
             self.ok = True
         except Exception as e:  # noqa: BLE001 -- NVML missing is reported, not fatal
             self.err = repr(e)
@@ -151,7 +155,9 @@ class ClockSampler:
         s = sorted(self.samples)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None,
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(s),
-                "power_w_max": max(self.power) if self.power else None}
+                "power_w_max": max(self.power) if self.power else None,
+                "power_w_mean": sum(self.power) / len(self.power) if self.power else None,
+                "power_limit_w": self.tdp_w}
 
 
 def physical_index(local):
@@ -673,6 +679,12 @@ def run_ours(args, W):
             "gpu_launches": r.launches * args.steps, "gpu_launches_per_step": r.launches,
             "roofline": B.roofline(W, m, args.mode)}
     line.update(m["extra"])
+    if clocks.get("power_limit_w"):
+        # the paper's energy-to-solution convention (Table 3): TDP x run time; beside it the power NVML
+        # reported while the timed regions ran (device-resident and e2e legs together)
+        line["energy"] = {"convention": "TDP x time (paper Table 3)", "tdp_w": clocks["power_limit_w"],
+                          "joules_per_step_tdp": clocks["power_limit_w"] * m["ms"] * 1e-3 * world,
+                          "joules_per_step_at_mean_sampled_power": (clocks["power_w_mean"] or 0.0) * m["ms"] * 1e-3 * world}
     if args.shard == "rows":
         # per-rank step times (a block's rows cost the same everywhere: the spread is the load imbalance of the cut)
         t = torch.zeros(world, dtype=torch.float64, device="cuda")

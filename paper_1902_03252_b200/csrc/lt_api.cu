@@ -542,7 +542,7 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   }
   const int quads_per_row = (nx + 3) / 4;
   {
-    long long blocks = ((long long)quads_per_row * ny + 255) / 256;
+    long long blocks = ((long long)quads_per_row * ny + LT_QUADS_PER_THREAD * 256 - 1) / (LT_QUADS_PER_THREAD * 256);
     const long long cap = (long long)dev.sms * 8;
     if (blocks > cap) blocks = cap;
     LT_CUDA(launch_dependent(lt_quad_list_kernel, (int)blocks, 256, 0, st, (const unsigned char*)flags, nx, ny, quads_per_row,

@@ -91,7 +91,7 @@ __device__ __forceinline__ void lt_cell_exact(const double2* __restrict__ grad, 
                    max_hits, n_hits);
 }
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 2)
 lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_min, double dx, int nx, int ny,
                       double dls_dos, const double2* __restrict__ sources, int n_sources, int n_strips, int n_items,
                       LtImageHit* __restrict__ hits, int max_hits, int* __restrict__ n_hits) {
@@ -123,11 +123,18 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
       double2 b = lt_node_beta(__ldg(col + (size_t)j_begin * nx), i, j_begin, x_min, y_min, dx, dls_dos, t1, t2);
       float pfx = (float)b.x, pfy = (float)b.y;
       float prx = __shfl_down_sync(0xffffffffu, pfx, 1), pry = __shfl_down_sync(0xffffffffu, pfy, 1);
-      for (int j0 = j_begin; j0 < j_end; j0 += LT_FI_ROWS) {
-        double2 g[LT_FI_ROWS];
+      double2 g[LT_FI_ROWS], g_next[LT_FI_ROWS];
 #pragma unroll
-        for (int r = 0; r < LT_FI_ROWS; ++r)                               // node rows j0 + 1 .. j0 + 4, clamped to the map
-          g[r] = __ldg(col + (size_t)min(j0 + r + 1, ny - 1) * nx);
+      for (int r = 0; r < LT_FI_ROWS; ++r)                                 // node rows j_begin + 1 .. + 4, clamped to the map
+        g_next[r] = __ldg(col + (size_t)min(j_begin + r + 1, ny - 1) * nx);
+      for (int j0 = j_begin; j0 < j_end; j0 += LT_FI_ROWS) {
+#pragma unroll
+        for (int r = 0; r < LT_FI_ROWS; ++r) {
+          g[r] = g_next[r];
+          // the rows of the NEXT group are requested before this group is worked on: the kernel is bound by the latency
+          // of a row segment, not by arithmetic (past the block's end the clamped row is loaded and dropped)
+          g_next[r] = __ldg(col + (size_t)min(j0 + LT_FI_ROWS + r + 1, ny - 1) * nx);
+        }
         float lo_x[LT_FI_ROWS], hi_x[LT_FI_ROWS], lo_y[LT_FI_ROWS], hi_y[LT_FI_ROWS];
         float wlo_x = INFINITY, whi_x = -INFINITY, wlo_y = INFINITY, whi_y = -INFINITY;
 #pragma unroll
@@ -166,25 +173,32 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
           whi_y = fmaxf(whi_y, __shfl_xor_sync(0xffffffffu, whi_y, o));
         }
         // warp-level culling: 32 sources at a time, one per lane, against the warp's box; survivors per cell
-        for (int k0 = 0; k0 < cnt; k0 += 32) {
-          const LtSrcBox bw = box[k0 + lane];        // entries beyond cnt are boxes nothing can hit
-          unsigned m = __ballot_sync(0xffffffffu, (bw.x_ru >= wlo_x) & (bw.x_rd <= whi_x) & (bw.y_ru >= wlo_y) & (bw.y_rd <= whi_y));
-          while (m) {
-            const int k = k0 + __ffs(m) - 1;
-            m &= m - 1;
-            const LtSrcBox sb = box[k];
-            // most survivors of the warp's box are in no lane's box: one vote instead of four cell tests per lane
-            if (!__any_sync(0xffffffffu, (sb.x_ru >= llo_x) & (sb.x_rd <= lhi_x) & (sb.y_ru >= llo_y) & (sb.y_rd <= lhi_y))) continue;
-            unsigned cells = 0;        // the lane's cells whose box the source can be in
+        for (int k0 = 0; k0 < cnt; k0 += 64) {       // two sets of 32 sources per step: their loads and votes overlap
+          const LtSrcBox bwa = box[k0 + lane], bwb = box[(k0 + 32 + lane) & (LT_SRC_CHUNK - 1)];   // beyond cnt: boxes nothing can hit
+          const unsigned ma = __ballot_sync(0xffffffffu, (bwa.x_ru >= wlo_x) & (bwa.x_rd <= whi_x) & (bwa.y_ru >= wlo_y) & (bwa.y_rd <= whi_y));
+          const unsigned mb = k0 + 32 < cnt
+              ? __ballot_sync(0xffffffffu, (bwb.x_ru >= wlo_x) & (bwb.x_rd <= whi_x) & (bwb.y_ru >= wlo_y) & (bwb.y_rd <= whi_y)) : 0u;
+#pragma unroll 1
+          for (int half = 0; half < 2; ++half) {
+            unsigned m = half ? mb : ma;
+            const int kb = k0 + 32 * half;
+            while (m) {
+              const int k = kb + __ffs(m) - 1;
+              m &= m - 1;
+              const LtSrcBox sb = box[k];
+              // most survivors of the warp's box are in no lane's box: one vote instead of four cell tests per lane
+              if (!__any_sync(0xffffffffu, (sb.x_ru >= llo_x) & (sb.x_rd <= lhi_x) & (sb.y_ru >= llo_y) & (sb.y_rd <= lhi_y))) continue;
+              unsigned cells = 0;        // the lane's cells whose box the source can be in
 #pragma unroll
-            for (int r = 0; r < LT_FI_ROWS; ++r)
-              // conservative: P in [lo, hi] in exact arithmetic implies this test passes
-              if ((sb.x_ru >= lo_x[r]) & (sb.x_rd <= hi_x[r]) & (sb.y_ru >= lo_y[r]) & (sb.y_rd <= hi_y[r])) cells |= 1u << r;
-            while (cells) {
-              const int r = __ffs(cells) - 1;
-              cells &= cells - 1;
-              lt_cell_exact(grad, i, j0 + r, nx, x_min, y_min, dx, dls_dos, src[k].x, src[k].y, base + k, hits, max_hits,
-                            n_hits);
+              for (int r = 0; r < LT_FI_ROWS; ++r)
+                // conservative: P in [lo, hi] in exact arithmetic implies this test passes
+                if ((sb.x_ru >= lo_x[r]) & (sb.x_rd <= hi_x[r]) & (sb.y_ru >= lo_y[r]) & (sb.y_rd <= hi_y[r])) cells |= 1u << r;
+              while (cells) {
+                const int r = __ffs(cells) - 1;
+                cells &= cells - 1;
+                lt_cell_exact(grad, i, j0 + r, nx, x_min, y_min, dx, dls_dos, src[k].x, src[k].y, base + k, hits, max_hits,
+                              n_hits);
+              }
             }
           }
         }

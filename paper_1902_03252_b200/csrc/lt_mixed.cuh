@@ -149,37 +149,65 @@ lt_flag_kernel(const float2* __restrict__ sp, int nx, int ny, LtMixedDev mp, uns
   }
 }
 
-// a8, part 3: compact list of the quads (j, iq) -> j * quads_per_row + iq that hold a flagged pixel.  One quad per thread,
-// warp-aggregated append (one atomic per warp and iteration); the order of the list is irrelevant because every quad is
-// recomputed independently.  Flag bytes are read with one 32-bit load where the quad is 4-byte aligned and inside the row.
+// a8, part 3: compact list of the quads (j, iq) -> j * quads_per_row + iq that hold a flagged pixel.  A CTA takes
+// LT_QUADS_PER_THREAD * 256 consecutive quads per iteration, LT_QUADS_PER_THREAD per thread (256 apart: coalesced, all
+// loads in flight together), and appends with ONE atomic per CTA and iteration (a warp scans the 32 segment counts) --
+// where nearly every quad is listed, an atomic per warp is a queue on one address (config 3: 131 000 of them, 92 us).
+// The order of the list is irrelevant because every quad is recomputed independently.  Flag bytes are read with one
+// 32-bit load where the quad is 4-byte aligned and inside the row.
+#define LT_QUADS_PER_THREAD 4
+__device__ __forceinline__ bool lt_quad_any(const unsigned char* __restrict__ flags, size_t q, size_t n_quads, int nx,
+                                            int quads_per_row) {
+  if (q >= n_quads) return false;
+  const size_t j = q / (size_t)quads_per_row;
+  const int i0 = (int)(q - j * (size_t)quads_per_row) * 4;
+  const size_t p = j * (size_t)nx + (size_t)i0;
+  if (i0 + 3 < nx && (p & 3) == 0) return *reinterpret_cast<const unsigned int*>(flags + p) != 0u;
+  bool any = false;
+  for (int k = 0; k < 4; ++k)
+    if (i0 + k < nx) any = any || flags[p + k] != 0;
+  return any;
+}
 __global__ void __launch_bounds__(256)
 lt_quad_list_kernel(const unsigned char* __restrict__ flags, int nx, int ny, int quads_per_row,
                     unsigned int* __restrict__ list, LtWsHeader* __restrict__ hdr) {
   lt_grid_dependency_wait();
-  const unsigned lane = threadIdx.x & 31;
+  const unsigned lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   const size_t n_quads = (size_t)quads_per_row * ny;
-  // whole warps iterate together so that the ballots see a full mask
-  for (size_t base = ((size_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u)); base < n_quads;
-       base += (size_t)gridDim.x * blockDim.x) {
-    const size_t q = base + lane;
-    bool any = false;
-    if (q < n_quads) {
-      const size_t j = q / (size_t)quads_per_row;
-      const int i0 = (int)(q - j * (size_t)quads_per_row) * 4;
-      const size_t p = j * (size_t)nx + (size_t)i0;
-      if (i0 + 3 < nx && (p & 3) == 0) {
-        any = *reinterpret_cast<const unsigned int*>(flags + p) != 0u;
-      } else {
-        for (int k = 0; k < 4; ++k)
-          if (i0 + k < nx) any = any || flags[p + k] != 0;
+  constexpr size_t TILE = (size_t)LT_QUADS_PER_THREAD * 256;
+  __shared__ unsigned int seg_base[LT_QUADS_PER_THREAD * 8];          // segment s = k * 8 + warp: 32 quads of sub-tile k
+  static_assert(LT_QUADS_PER_THREAD * 8 == 32, "one segment per lane of warp 0");
+  // whole CTAs iterate together so that the ballots see a full mask and the barriers are reached by every thread
+  for (size_t base = (size_t)blockIdx.x * TILE; base < n_quads; base += (size_t)gridDim.x * TILE) {
+    bool any[LT_QUADS_PER_THREAD];
+    unsigned m[LT_QUADS_PER_THREAD];
+#pragma unroll
+    for (int k = 0; k < LT_QUADS_PER_THREAD; ++k)
+      any[k] = lt_quad_any(flags, base + (size_t)k * 256 + threadIdx.x, n_quads, nx, quads_per_row);
+#pragma unroll
+    for (int k = 0; k < LT_QUADS_PER_THREAD; ++k) {
+      m[k] = __ballot_sync(0xffffffffu, any[k]);
+      if (lane == 0) seg_base[k * 8 + wrp] = (unsigned int)__popc(m[k]);
+    }
+    __syncthreads();
+    if (wrp == 0) {
+      const unsigned int cnt = seg_base[lane];
+      unsigned int incl = cnt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((int)lane >= o) incl += v;
       }
+      unsigned int cta_base = 0;
+      if (lane == 31 && incl) cta_base = atomicAdd(&hdr->list_count, incl);
+      cta_base = __shfl_sync(0xffffffffu, cta_base, 31);
+      seg_base[lane] = cta_base + incl - cnt;
     }
-    const unsigned m = __ballot_sync(0xffffffffu, any);
-    if (m) {
-      unsigned int warp_base = 0;
-      if (lane == 0) warp_base = atomicAdd(&hdr->list_count, (unsigned int)__popc(m));
-      warp_base = __shfl_sync(0xffffffffu, warp_base, 0);
-      if (any) list[warp_base + __popc(m & ((1u << lane) - 1u))] = (unsigned int)q;
-    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < LT_QUADS_PER_THREAD; ++k)
+      if (any[k])
+        list[seg_base[k * 8 + wrp] + __popc(m[k] & ((1u << lane) - 1u))] = (unsigned int)(base + (size_t)k * 256 + threadIdx.x);
+    __syncthreads();                                          // seg_base is rewritten by the next iteration
   }
 }
