@@ -61,8 +61,15 @@ __device__ __forceinline__ void lt_test_triangle(double Ax, double Ay, double Bx
   hits[slot] = h;
 }
 
+#ifndef LT_FI_ROWS
 #define LT_FI_ROWS 4            // rows per group
+#endif
+#ifndef LT_FI_BLOCK_ROWS
 #define LT_FI_BLOCK_ROWS 64     // cell rows per work item (one more node row is read to start it: 1.6 % of the traffic)
+#endif
+#ifndef LT_FI_MINB
+#define LT_FI_MINB 2
+#endif
 #define LT_FI_STRIP 31          // cell columns per strip
 
 // source-plane image of node (i, j), eq. 13: exactly the operations of the API's definition, so that the hot path (which
@@ -91,7 +98,7 @@ __device__ __forceinline__ void lt_cell_exact(const double2* __restrict__ grad, 
                    max_hits, n_hits);
 }
 
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256, LT_FI_MINB)
 lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_min, double dx, int nx, int ny,
                       double dls_dos, const double2* __restrict__ sources, int n_sources, int n_strips, int n_items,
                       LtImageHit* __restrict__ hits, int max_hits, int* __restrict__ n_hits) {
@@ -173,32 +180,25 @@ lt_find_images_kernel(const double2* __restrict__ grad, double x_min, double y_m
           whi_y = fmaxf(whi_y, __shfl_xor_sync(0xffffffffu, whi_y, o));
         }
         // warp-level culling: 32 sources at a time, one per lane, against the warp's box; survivors per cell
-        for (int k0 = 0; k0 < cnt; k0 += 64) {       // two sets of 32 sources per step: their loads and votes overlap
-          const LtSrcBox bwa = box[k0 + lane], bwb = box[(k0 + 32 + lane) & (LT_SRC_CHUNK - 1)];   // beyond cnt: boxes nothing can hit
-          const unsigned ma = __ballot_sync(0xffffffffu, (bwa.x_ru >= wlo_x) & (bwa.x_rd <= whi_x) & (bwa.y_ru >= wlo_y) & (bwa.y_rd <= whi_y));
-          const unsigned mb = k0 + 32 < cnt
-              ? __ballot_sync(0xffffffffu, (bwb.x_ru >= wlo_x) & (bwb.x_rd <= whi_x) & (bwb.y_ru >= wlo_y) & (bwb.y_rd <= whi_y)) : 0u;
-#pragma unroll 1
-          for (int half = 0; half < 2; ++half) {
-            unsigned m = half ? mb : ma;
-            const int kb = k0 + 32 * half;
-            while (m) {
-              const int k = kb + __ffs(m) - 1;
-              m &= m - 1;
-              const LtSrcBox sb = box[k];
-              // most survivors of the warp's box are in no lane's box: one vote instead of four cell tests per lane
-              if (!__any_sync(0xffffffffu, (sb.x_ru >= llo_x) & (sb.x_rd <= lhi_x) & (sb.y_ru >= llo_y) & (sb.y_rd <= lhi_y))) continue;
-              unsigned cells = 0;        // the lane's cells whose box the source can be in
+        for (int k0 = 0; k0 < cnt; k0 += 32) {
+          const LtSrcBox bw = box[k0 + lane];        // entries beyond cnt are boxes nothing can hit
+          unsigned m = __ballot_sync(0xffffffffu, (bw.x_ru >= wlo_x) & (bw.x_rd <= whi_x) & (bw.y_ru >= wlo_y) & (bw.y_rd <= whi_y));
+          while (m) {
+            const int k = k0 + __ffs(m) - 1;
+            m &= m - 1;
+            const LtSrcBox sb = box[k];
+            // most survivors of the warp's box are in no lane's box: one vote instead of four cell tests per lane
+            if (!__any_sync(0xffffffffu, (sb.x_ru >= llo_x) & (sb.x_rd <= lhi_x) & (sb.y_ru >= llo_y) & (sb.y_rd <= lhi_y))) continue;
+            unsigned cells = 0;        // the lane's cells whose box the source can be in
 #pragma unroll
-              for (int r = 0; r < LT_FI_ROWS; ++r)
-                // conservative: P in [lo, hi] in exact arithmetic implies this test passes
-                if ((sb.x_ru >= lo_x[r]) & (sb.x_rd <= hi_x[r]) & (sb.y_ru >= lo_y[r]) & (sb.y_rd <= hi_y[r])) cells |= 1u << r;
-              while (cells) {
-                const int r = __ffs(cells) - 1;
-                cells &= cells - 1;
-                lt_cell_exact(grad, i, j0 + r, nx, x_min, y_min, dx, dls_dos, src[k].x, src[k].y, base + k, hits, max_hits,
-                              n_hits);
-              }
+            for (int r = 0; r < LT_FI_ROWS; ++r)
+              // conservative: P in [lo, hi] in exact arithmetic implies this test passes
+              if ((sb.x_ru >= lo_x[r]) & (sb.x_rd <= hi_x[r]) & (sb.y_ru >= lo_y[r]) & (sb.y_rd <= hi_y[r])) cells |= 1u << r;
+            while (cells) {
+              const int r = __ffs(cells) - 1;
+              cells &= cells - 1;
+              lt_cell_exact(grad, i, j0 + r, nx, x_min, y_min, dx, dls_dos, src[k].x, src[k].y, base + k, hits, max_hits,
+                            n_hits);
             }
           }
         }
