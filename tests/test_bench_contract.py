@@ -95,3 +95,30 @@ def test_strong_scaling_arm_on_one_gpu():
     d = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][0])
     assert d["scaling"] == "strong" and d["config"]["parallelism"].startswith("rows/1")
     assert d["shard"]["rows_per_rank"] == [2048] and len(d["shard"]["ms_per_rank"]) == 1 and d["value"] > 1e10
+
+
+def test_parity_block_of_the_bench_line_on_cpu():
+    """bench.py's parity leg (oracle_parity) needs no GPU for its own logic: fed with the oracle's `double` map as the
+    "device" values it must report a tiny error that passes, with the sample it promises; fed with a map that is off by
+    2e-5 of max|alpha| in one pixel it must fail fp32's tolerance."""
+    import numpy as np
+    sys.path.insert(0, ROOT)
+    import bench
+    from oracle import lt_oracle as O
+    from paper_1902_03252_b200 import workloads
+    W = workloads.make(0)
+    i, j = bench.parity_sample(W)
+    assert len(i) == 20000 + 8 and i.min() >= 0 and i.max() < W.nx and j.max() < W.ny
+    g = O.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny, precision=O.DOUBLE)
+    got = g[j, i]
+    flags = np.zeros(len(i), np.uint8)
+    flags[:100] = 2
+    sampled = {"fp64": got, "fp32": got.astype(np.float32).astype(np.float64), "mixed": got.copy()}
+    p = bench.oracle_parity(W, sampled, flags, (3.26, 0.0104 / 0.03, 6.0, 0.3, 15.0))
+    assert p["fp64"]["pass"] and p["fp64"]["max_err_rel"] < 1e-13 and p["fp64"]["tol"] == 1e-12
+    assert p["fp32"]["pass"] and 1e-9 < p["fp32"]["max_err_rel"] < 1e-6 and p["fp32"]["n_sampled"] == len(i)
+    assert p["mixed"]["flagged_bit_equal_to_fp64_mode"] and p["mixed"]["n_flagged_in_sample"] == 100
+    bad = dict(sampled)
+    bad["fp32"] = got.copy()
+    bad["fp32"][7, 1] += 2e-5 * np.abs(g).max()
+    assert not bench.oracle_parity(W, bad, flags, (3.26, 0.0104 / 0.03, 6.0, 0.3, 15.0))["fp32"]["pass"]
