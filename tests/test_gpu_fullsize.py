@@ -61,15 +61,25 @@ def _run(torch, lt, W, mode, mixed=None):
 
 def _fullgrid(env, cfg):
     torch, lt, O, S = env
-    W = workloads.make(cfg)
-    ref = _oracle_map(O, W)
+    if cfg == "sie":
+        W, mixed = workloads.make_sie("paper"), SIE_MIXED
+        ref = S.gradient_grid(W.lenses, W.x_min, W.y_min, W.dx, W.nx, W.ny)
+    else:
+        W, mixed = workloads.make(cfg), None
+        ref = _oracle_map(O, W)
     s = np.abs(ref).reshape(-1, 2).max(axis=0)
     res = {}
     for mode, name in ((lt.LT_FP64, "fp64"), (lt.LT_FP32, "fp32"), (lt.LT_MIXED, "mixed")):
-        out = _run(torch, lt, W, mode)[0].cpu().numpy().astype(np.float64)
+        out, ws = _run(torch, lt, W, mode, mixed=mixed if mode == lt.LT_MIXED else None)
+        out = out.cpu().numpy().astype(np.float64)
         e = np.abs(out - ref).reshape(-1, 2)
+        if cfg == "sie" and mode == lt.LT_FP32:      # R10: fp32 is gated outside the rule's DP patches (reported inside)
+            keep = (O.mixed_flags(ref.astype(np.float32), S.as_rule_catalogue(W.lenses), W.x_min, W.y_min, W.dx,
+                                  mixed=SIE_MIXED) & 1) == 0
+            print("sie fp32 inside the DP patches (reported, not gated): max", (e[~keep.reshape(-1)].max(axis=0) / s).max())
+            e = e[keep.reshape(-1)]
         res[name] = ((e.max(axis=0) / s).max(), (np.sqrt((e ** 2).mean(axis=0)) / s).max())
-        del out, e
+        del out, e, ws
     print(W.name, "every pixel vs long-double oracle:", " | ".join("%s max %.3e rms %.3e" % (k, v[0], v[1]) for k, v in res.items()))
     assert res["fp64"][0] < TOL_F64 and res["fp32"][0] < TOL_F32 and res["mixed"][0] < TOL_F32
 
@@ -82,6 +92,12 @@ def test_every_pixel_against_the_oracle(env, cfg):
 @pytest.mark.skipif(os.environ.get("LT_FULLGRID_CFG3") != "1", reason="~7 minutes of oracle time; set LT_FULLGRID_CFG3=1")
 def test_every_pixel_against_the_oracle_cfg3(env):
     _fullgrid(env, 3)
+
+
+@pytest.mark.skipif(os.environ.get("LT_FULLGRID_SIE") != "1", reason="minutes of oracle time; set LT_FULLGRID_SIE=1")
+def test_every_pixel_against_the_oracle_sie_benchmark(env):
+    """the paper-like benchmark, 45.3 M pixels x 702 halos, paper constants for the mixed mode"""
+    _fullgrid(env, "sie")
 
 
 def _rule_catalogue(S, W):
