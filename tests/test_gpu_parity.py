@@ -93,6 +93,26 @@ def test_launch_configurations_agree(env, ppt64, ppt32, chunk):
     assert _err(a, ref) < TOL_F64 and _err(b, ref) < TOL_F32
 
 
+def test_oversized_chunk_request_is_clamped(env):
+    """lt_set_tuning(chunk64 = chunk32 = 65536) with 4096 lenses: the wanted chunk exceeds what fits beside each kernel's
+    own static shared memory (the range-reduction tables) under the opt-in limit; the library clamps it per kernel instead
+    of failing the launch, and the map does not change (fp64 bit-equal, all three modes run)."""
+    torch, lt, O = env
+    L = workloads.random_catalogue(11, 4096, L=80.0)
+    W = workloads.Workload("many", L, -80.0, -80.0, 2.5, 64, 40, 11)
+    base = _gpu_map(torch, lt, W, lt.LT_FP64)
+    try:
+        lt.lt_set_tuning(0, 0, 65536, 65536, 0)
+        a = _gpu_map(torch, lt, W, lt.LT_FP64)
+        b = _gpu_map(torch, lt, W, lt.LT_FP32)
+        m = _gpu_map(torch, lt, W, lt.LT_MIXED)
+    finally:
+        lt.lt_set_tuning()
+    assert np.array_equal(a, base)
+    s = np.abs(base).max()
+    assert np.abs(b.astype(np.float64) - base).max() / s < TOL_F32 and np.abs(m - base).max() / s < TOL_F32
+
+
 @pytest.mark.parametrize("nx,ny,ctas", [(1500, 1111, 0), (1027, 2049, 1), (4096, 300, 2), (129, 4100, 0)])
 def test_wave_split_covers_every_pixel_once(env, nx, ny, ctas):
     """The launch plan (whole waves of the widest variant, ragged rest to the finer ones: lt_api.cu launch_waves)
