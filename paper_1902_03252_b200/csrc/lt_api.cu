@@ -382,21 +382,19 @@ int launch_quads(const typename Rec64<M>::type* l64, const LtTables<double>* t64
   return LT_OK;
 }
 
-template <class M, bool FROM_LIST>
-int launch_list(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, const unsigned int* list, const LtWsHeader* hdr,
-                const double2* points, long long n_points, long long max_work, double2* out, const DeviceInfo& d,
-                cudaStream_t st) {
+template <class M>
+int launch_points(const typename Rec64<M>::type* l64, const LtTables<double>* t64, int n_lens, const double2* points,
+                  long long n_points, double2* out, const DeviceInfo& d, cudaStream_t st) {
   int chunk = 1, grid = 1;
   const int wanted = g_tuning.chunk64;
-  int rc = pick_chunk(lt_grad_list_f64_kernel<M, FROM_LIST>, a.n_lens, wanted > 0 ? wanted : kDefaultChunk64,
+  int rc = pick_chunk(lt_grad_points_f64_kernel<M>, n_lens, wanted > 0 ? wanted : kDefaultChunk64,
                       sizeof(typename Rec64<M>::type), d, chunk);
   if (rc != LT_OK) return rc;
   const size_t smem = (size_t)chunk * sizeof(typename Rec64<M>::type);
-  rc = grid_for(lt_grad_list_f64_kernel<M, FROM_LIST>, smem, (max_work + LT_THREADS - 1) / LT_THREADS, d, grid);
+  rc = grid_for(lt_grad_points_f64_kernel<M>, smem, (n_points + LT_THREADS - 1) / LT_THREADS, d, grid);
   if (rc != LT_OK) return rc;
-  KernelEvents ke(st, FROM_LIST);
-  LT_CUDA(launch_dependent(lt_grad_list_f64_kernel<M, FROM_LIST>, grid, LT_THREADS, smem, st, l64, t64, a.n_lens, chunk,
-                           a.x_min, a.y_min, a.dx, a.nx, list, hdr, points, n_points, out));
+  LT_CUDA(launch_dependent(lt_grad_points_f64_kernel<M>, grid, LT_THREADS, smem, st, l64, t64, n_lens, chunk, points,
+                           n_points, out));
   ++g_launches;
   return LT_OK;
 }
@@ -581,11 +579,9 @@ int gradient_points_impl(const void* d_lenses, int n_lens, const double* d_point
     ++g_launches;
     return LT_OK;
   }
-  return launch_list<M, false>(reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
-                            reinterpret_cast<const LtTables<double>*>(ws + L.tab64), a, nullptr,
-                            reinterpret_cast<const LtWsHeader*>(ws + L.header),
-                            reinterpret_cast<const double2*>(d_points), n_points, n_points,
-                            reinterpret_cast<double2*>(d_out), dev, st);
+  return launch_points<M>(reinterpret_cast<const typename Rec64<M>::type*>(ws + L.lens64),
+                          reinterpret_cast<const LtTables<double>*>(ws + L.tab64), n_lens,
+                          reinterpret_cast<const double2*>(d_points), n_points, reinterpret_cast<double2*>(d_out), dev, st);
 }
 
 template <class M>

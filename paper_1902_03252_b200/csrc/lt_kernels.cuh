@@ -1,5 +1,5 @@
 // lt_kernels.cuh -- device kernels of the gradient-map path: per-lens precompute, the fp64 and
-// fp32 grid kernels, and the fp64 list kernel that serves the mixed-precision recompute (a9) and lt_gradient_points.
+// fp32 grid kernels, the fp64 quad kernel of the mixed-precision recompute (a9) and the kernels of lt_gradient_points.
 //
 // Mapping: data parallelism over pixels only.  A CTA owns tiles of TILE_W x TILE_H
 // pixels (a warp = one row segment, each thread PPT pixels strided by 32 in x so that every store instruction of a
@@ -349,42 +349,28 @@ lt_grad_f32_plain_kernel(const typename M::Raw* __restrict__ raw, const typename
   }
 }
 
-// ------------------------------------------------------------------------------------------------ fp64 list kernel
-// Pixels taken from (a) the compacted list of flagged pixel indices of the mixed rule (a9; count read from the
-// workspace header on the device, no host round trip) or (b) an array of arbitrary points.  Uses the same
-// interact_sky in the same lens order as the fp64 grid kernel: identical bits for identical pixels.
-// Groups of 4 * 256 entries, 4 per thread (entries 256 apart, so list reads stay coalesced); a rest of at most one
-// 256-entry group per CTA after the whole waves runs one entry per thread (the count is only known on the device, so
-// the split is made here, not on the host).
-template <class M, bool FROM_LIST, int PPT>
-__device__ __forceinline__ void lt_list_group(const typename M::template Rec<double>::type* __restrict__ lens,
-                                              const typename M::template Rec<double>::type* sl,
-                                              const LtTables<double>& tab, int n_lens, int chunk, bool single,
-                                              double x_min, double y_min, double dx, int nx,
-                                              const unsigned int* __restrict__ list,
-                                              const double2* __restrict__ points, long long first, long long total,
-                                              double2* __restrict__ out) {
+// ------------------------------------------------------------------------------------------------ fp64 point-list kernel
+// lt_gradient_points with more than a few thousand points: the gradient at an array of arbitrary points, one thread per
+// point.  Uses the same interact_abs in the same lens order as the fp64 grid kernel: for a point that is a grid node,
+// identical bits.  Groups of 4 * 256 points, 4 per thread (256 apart, so the reads stay coalesced); a rest of at most one
+// 256-point group per CTA after the whole waves runs one point per thread.
+template <class M, int PPT>
+__device__ __forceinline__ void lt_points_group(const typename M::template Rec<double>::type* __restrict__ lens,
+                                                const typename M::template Rec<double>::type* sl,
+                                                const LtTables<double>& tab, int n_lens, int chunk, bool single,
+                                                const double2* __restrict__ points, long long first, long long total,
+                                                double2* __restrict__ out) {
   double t1[PPT], t2[PPT], G1[PPT], G2[PPT];
-  size_t dst[PPT];
   bool live[PPT];
 #pragma unroll
   for (int p = 0; p < PPT; ++p) {
     const long long t = first + (long long)p * LT_THREADS + threadIdx.x;
     live[p] = t < total;
-    t1[p] = 0.0; t2[p] = 0.0; dst[p] = 0; G1[p] = 0.0; G2[p] = 0.0;
+    t1[p] = 0.0; t2[p] = 0.0; G1[p] = 0.0; G2[p] = 0.0;
     if (live[p]) {
-      if (FROM_LIST) {
-        const unsigned int pix = list[t];
-        const int j = (int)(pix / (unsigned int)nx), i = (int)(pix - (unsigned int)j * (unsigned int)nx);
-        t1[p] = __dadd_rn(x_min, __dmul_rn((double)i, dx));
-        t2[p] = __dadd_rn(y_min, __dmul_rn((double)j, dx));
-        dst[p] = pix;
-      } else {
-        const double2 pt = points[t];
-        t1[p] = pt.x;
-        t2[p] = pt.y;
-        dst[p] = (size_t)t;
-      }
+      const double2 pt = points[t];
+      t1[p] = pt.x;
+      t2[p] = pt.y;
     }
   }
   for (int base = 0; base < n_lens; base += chunk) {
@@ -405,15 +391,14 @@ __device__ __forceinline__ void lt_list_group(const typename M::template Rec<dou
   }
 #pragma unroll
   for (int p = 0; p < PPT; ++p)
-    if (live[p]) out[dst[p]] = make_double2(G1[p], G2[p]);
+    if (live[p]) out[first + (long long)p * LT_THREADS + threadIdx.x] = make_double2(G1[p], G2[p]);
 }
 
-template <class M, bool FROM_LIST>
+template <class M>
 __global__ void __launch_bounds__(LT_THREADS, 2)
-lt_grad_list_f64_kernel(const typename M::template Rec<double>::type* __restrict__ lens, const LtTables<double>* __restrict__ tables,
-                        int n_lens, int chunk, double x_min, double y_min, double dx, int nx,
-                        const unsigned int* __restrict__ list, const LtWsHeader* __restrict__ hdr,
-                        const double2* __restrict__ points, long long n_points, double2* __restrict__ out) {
+lt_grad_points_f64_kernel(const typename M::template Rec<double>::type* __restrict__ lens, const LtTables<double>* __restrict__ tables,
+                          int n_lens, int chunk, const double2* __restrict__ points, long long n_points,
+                          double2* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char lt_smem[];
   typedef typename M::template Rec<double>::type Rec;
   __shared__ LtTables<double> tab;
@@ -421,7 +406,7 @@ lt_grad_list_f64_kernel(const typename M::template Rec<double>::type* __restrict
   lt_grid_dependency_wait();
   if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
   __syncthreads();
-  const long long total = FROM_LIST ? (long long)hdr->list_count : n_points;
+  const long long total = n_points;
   const bool single = n_lens <= chunk;
   if (single) {
     lt_copy16(sl, lens, n_lens * (int)(sizeof(Rec) / 16));
@@ -429,27 +414,25 @@ lt_grad_list_f64_kernel(const typename M::template Rec<double>::type* __restrict
   }
   constexpr int WIDE = 4;
   const long long per_wave = (long long)gridDim.x * (WIDE * LT_THREADS);
-  long long n_wide = total / per_wave * gridDim.x;                  // groups of WIDE * 256 entries: whole waves
+  long long n_wide = total / per_wave * gridDim.x;                  // groups of WIDE * 256 points: whole waves
   long long rest0 = n_wide * (WIDE * LT_THREADS);
   if (total - rest0 > (long long)gridDim.x * LT_THREADS) {          // more than one narrow group per CTA left:
     n_wide = (total + WIDE * LT_THREADS - 1) / (WIDE * LT_THREADS); // a ragged wide wave is cheaper than narrow rounds
     rest0 = total;
   }
   for (long long g = blockIdx.x; g < n_wide; g += gridDim.x)
-    lt_list_group<M, FROM_LIST, WIDE>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
-                                   g * (WIDE * LT_THREADS), total, out);
+    lt_points_group<M, WIDE>(lens, sl, tab, n_lens, chunk, single, points, g * (WIDE * LT_THREADS), total, out);
   const long long n_rest = (total - rest0 + LT_THREADS - 1) / LT_THREADS;   // <= gridDim.x
   for (long long g = blockIdx.x; g < n_rest; g += gridDim.x)
-    lt_list_group<M, FROM_LIST, 1>(lens, sl, tab, n_lens, chunk, single, x_min, y_min, dx, nx, list, points,
-                                rest0 + g * LT_THREADS, total, out);
+    lt_points_group<M, 1>(lens, sl, tab, n_lens, chunk, single, points, rest0 + g * LT_THREADS, total, out);
 }
 
 // ------------------------------------------------------------------------------------------------ fp64 quad kernel (a9)
 // The fp64 pass of the mixed mode.  Work list: the quads of lt_quad_list_kernel (lt_mixed.cuh), count read from the
 // workspace header on the device (no host round trip).  A thread owns one quad = four neighbouring pixels of a row, so
 // its lens loop is the grid kernel's: one row term per lens shared by four interact_abs calls, same operations in the
-// same order -- identical bits for identical pixels at the grid kernel's instruction count (the per-pixel list kernel
-// below forms the row terms once per pixel).  All four pixels are recomputed, the flagged ones are stored.
+// same order -- identical bits for identical pixels at the grid kernel's instruction count (the per-point kernel
+// above forms the row terms once per pixel).  All four pixels are recomputed, the flagged ones are stored.
 template <class M>
 __global__ void __launch_bounds__(LT_THREADS, 2)
 lt_grad_quads_f64_kernel(const typename M::template Rec<double>::type* __restrict__ lens,
