@@ -104,7 +104,7 @@ typedef struct {               /* written by lt_chi2 (device memory, 32 bytes)  
 
 typedef struct {               /* filled by lt_mixed_last_stats */
   long long n_pixels;          /* -1: not recorded (the caller knows nx*ny)                                      */
-  long long n_flagged;         /* pixels recomputed in double precision = patch OR eq.25 OR eq.28                */
+  long long n_flagged;         /* pixels that carry double precision values = patch OR eq.25 OR eq.28             */
   long long n_patch, n_eq25, n_eq28;   /* pixels with the respective bit set (not exclusive)                     */
 } lt_mixed_stats;
 
@@ -119,7 +119,8 @@ size_t lt_workspace_bytes(int n_lens, int nx, int ny, lt_precision mode);
 /*
  * The hot path.  Enqueues on cuda_stream: the per-lens precompute kernel, the gradient kernel
  * (a2-a7) in the requested precision and, for LT_MIXED, the patch/flag/compaction kernels (a8) and the fp64
- * recompute of the flagged pixels (a9).  Asynchronous; returns after the launches.
+ * recompute of the flagged pixels (a9; done in row quads -- four neighbouring pixels of a row that hold a flagged pixel are
+ * recomputed together, only the flagged ones are stored).  Asynchronous; returns after the launches.
  *   d_lenses       device, n_lens lt_lens structs (= a contiguous [n_lens,7] fp64 array); read only
  *   mixed_or_null  host pointer; NULL = lt_mixed_defaults; ignored unless mode == LT_MIXED
  *   d_out_grad     device, nx*ny*2 elements (type per mode, see above); fully overwritten
@@ -172,7 +173,7 @@ int lt_gradient_grid_nfw_host(const lt_nfw_lens* h_lenses, int n_lens,
                               void* h_out_grad, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
- * Gradient at an arbitrary list of points (the a9 kernel exposed; used for sampled parity at full size and for
+ * Gradient at an arbitrary list of points (the per-lens arithmetic of a3-a6 exposed; used for sampled parity at full size and for
  * image positions).  d_points: n_points*2 doubles (theta_1, theta_2 interleaved); d_out: n_points*2 doubles.
  * fp64 only.  Same workspace rule with nx = ny = 1.  Lists of more than 4096 points run one thread per point and return,
  * for a point that is a grid node, the bits of lt_gradient_grid's LT_FP64 map.  Shorter lists (the image positions of
