@@ -271,7 +271,9 @@ int lt_chi2(const double* d_theta_obs, const double* d_sigma, const int* d_offse
  * programmatic-dependent-launch attribute, bit 4 = LT_FP32 and the first step of LT_MIXED run the
  * paper's plain SP version, "identical up to the change in precision": pixel coordinates, lens centres and
  * their difference in fp32, instead of the tile-centre coordinates of DESIGN.md section 5 -- a measurement variant
- * for the calibration of the mixed rule (what the centre patches of P:284 are for), not a mode.  Results do not depend on
+ * for the calibration of the mixed rule (what the centre patches of P:284 are for), not a mode; bit 5 = the fp64 kernels
+ * stage the lens records in shared memory always, instead of reading them from the constant bank where the call allows it
+ * (DESIGN.md section 6).  Results do not depend on
  * any of the others except that the fp32 tile centre moves with the pixels per thread of the launch
  * that owns the pixel.  Returns LT_ERR_BAD_SIZE on a negative value.
  * Thread safety: the knobs are independent atomics; a launch racing this call sees each knob either old or new.  They

@@ -35,7 +35,7 @@ thread_local int g_last_cuda_error = 0;
 // that races lt_set_tuning sees every knob either old or new (the knobs are independent of one another)
 struct Tuning {
   std::atomic<int> ppt64{0}, ppt32{0}, chunk64{0}, chunk32{0}, ctas_per_sm{0}, single_launch{0}, staged_host_output{0},
-      points_per_thread{0}, no_dependent_launch{0}, plain_sp{0};
+      points_per_thread{0}, no_dependent_launch{0}, plain_sp{0}, no_const_records{0};
 };
 Tuning g_tuning;
 thread_local cudaEvent_t g_ev_start = nullptr, g_ev_stop = nullptr;   // lt_set_kernel_events
@@ -231,6 +231,8 @@ struct GridArgs {
   int n_lens;
   double x_min, y_min, dx;
   int nx, ny;
+  double2* staging = nullptr;   // device buffer of nx*ny double2 the host entry points own: where a map that goes straight
+                                // into pinned host memory keeps its partial sums between launches (constant-bank records)
 };
 
 // Launch plan shared by the fp64 and fp32 grid kernels.  All tiles cost the same, so a persistent grid of R resident CTAs
@@ -281,18 +283,110 @@ int launch_f64_ppt(const typename Rec64<M>::type* l64, const LtTables<double>* t
   ++g_launches;
   return LT_OK;
 }
+// ---- lens records in the constant bank (lt_kernels.cuh: lt_grad_f64_const_kernel) --------------------------------------
+// One slot of __constant__ memory per device (= per context: the library is one module).  Whoever launches a kernel that
+// reads the slot holds `mu` while it enqueues: [wait for the slot's last reader if that was another stream] copy the
+// records in (device to device, stream-ordered), launch, record `ev`.  Nothing blocks the host; two streams that both use
+// the slot are ordered on it (two maps at once would not overlap anyway: each fills the GPU).
+struct ConstSlot {
+  std::mutex mu;
+  cudaEvent_t ev = nullptr;
+  cudaStream_t last = nullptr;
+  bool used = false;
+};
+ConstSlot g_const_slot[64];
+
+// May this call use the slot?  Not while the stream is being captured into a graph (a replay could not be ordered against
+// other users of the slot), not when lt_set_tuning switched it off, not beyond 64 devices.  A catalogue that needs several
+// slot-loads is accumulated over launches: in `out` if that is device memory, else in the caller's device staging buffer
+// with only the last launch writing to `out` (a map that goes straight into pinned host memory crosses PCIe once).
+bool const_records_ok(cudaStream_t st, const DeviceInfo& d, const void* out, const void* staging, int n_lens,
+                      size_t rec_bytes) {
+  if (g_tuning.no_const_records || d.device < 0 || d.device >= 64 || n_lens < 1) return false;
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+    (void)cudaGetLastError();
+    return false;
+  }
+  if ((size_t)n_lens * rec_bytes > LT_CONST_SLOT_BYTES && !staging) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, out) != cudaSuccess || at.type != cudaMemoryTypeDevice) {
+      (void)cudaGetLastError();
+      return false;
+    }
+  }
+  return true;
+}
+
+// fn(cnt, acc, dst): enqueue the kernel for the `cnt` records now in the slot, continuing the sums in `acc` (null: start
+// from zero) and storing to `dst`
+template <class Rec, class Fn>
+int with_const_records(const Rec* d_records, int n_lens, const DeviceInfo& d, cudaStream_t st, double2* out, double2* staging,
+                       Fn fn) {
+  ConstSlot& slot = g_const_slot[d.device];
+  std::lock_guard<std::mutex> lock(slot.mu);
+  if (!slot.ev) LT_CUDA(cudaEventCreateWithFlags(&slot.ev, cudaEventDisableTiming));
+  if (slot.used && slot.last != st) LT_CUDA(cudaStreamWaitEvent(st, slot.ev, 0));
+  const int per = (int)(LT_CONST_SLOT_BYTES / sizeof(Rec));
+  int rc = LT_OK;
+  for (int base = 0; base < n_lens && rc == LT_OK; base += per) {
+    const int cnt = n_lens - base < per ? n_lens - base : per;
+    LT_CUDA(cudaMemcpyToSymbolAsync(lt_const_slot, d_records + base, (size_t)cnt * sizeof(Rec), 0, cudaMemcpyDeviceToDevice, st));
+    // partial sums live in `between` (the staging buffer if there is one, else `out` itself); the last launch stores to `out`
+    double2* between = staging ? staging : out;
+    const bool last = base + cnt >= n_lens;
+    rc = fn(cnt, base > 0 ? (const double2*)between : (const double2*)nullptr, last ? out : between);
+  }
+  LT_CUDA(cudaEventRecord(slot.ev, st));     // also after a failed launch: the copies are in the stream
+  slot.last = st;
+  slot.used = true;
+  return rc;
+}
+
+// the 4-pixel main launch over tiles [begin, end) with the records in the constant bank
+template <class M>
+int launch_f64_const(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
+                     const DeviceInfo& d, cudaStream_t st, int tiles_x, long long begin, long long end, long long* resident) {
+  if (resident) return resident_ctas(lt_grad_f64_const_kernel<M, true>, 0, d, *resident);
+  int grid = 1;
+  const int rc = grid_for(lt_grad_f64_const_kernel<M, true>, 0, end - begin, d, grid);
+  if (rc != LT_OK) return rc;
+  long long r2 = 0;   // (opts the second instantiation in; same resources)
+  if (a.staging) {
+    const int rc2 = resident_ctas(lt_grad_f64_const_kernel<M, false>, 0, d, r2);
+    if (rc2 != LT_OK) return rc2;
+  }
+  return with_const_records(l64, a.n_lens, d, st, out, a.staging, [&](int cnt, const double2* acc, double2* dst) -> int {
+    if (a.staging)      // partial sums in the staging buffer, the last launch stores to `out` (pinned host memory)
+      LT_CUDA(launch_dependent(lt_grad_f64_const_kernel<M, false>, grid, LT_THREADS, 0, st, t64, cnt, acc, a.x_min, a.y_min,
+                               a.dx, a.nx, a.ny, tiles_x, (int)begin, (int)end, dst));
+    else                // in place
+      LT_CUDA(launch_dependent(lt_grad_f64_const_kernel<M, true>, grid, LT_THREADS, 0, st, t64, cnt, acc ? 1 : 0, a.x_min,
+                               a.y_min, a.dx, a.nx, a.ny, tiles_x, (int)begin, (int)end, dst));
+    ++g_launches;
+    return LT_OK;
+  });
+}
+
 template <class M>
 int launch_f64(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, double2* out,
                const DeviceInfo& d, cudaStream_t st, bool hook = true) {
   // 4 pixels per thread (4 independent chains, lens record loaded once per 4 interactions) at <= 128 registers, two
   // CTAs per SM; fewer pixels per thread for the ragged rest and for grids too small to give every SM two tiles
+  // The 4-pixel launch reads its records from the constant bank where it may (const_records_ok); the ragged rest and
+  // small grids keep the shared-memory kernels (they loop over the whole catalogue in one launch, on tiles of their own).
   KernelEvents ke(st, hook);
+  const bool cb = M::kConstRecords && const_records_ok(st, d, out, a.staging, a.n_lens, sizeof(typename Rec64<M>::type));
   return launch_waves(pick_ppt(g_tuning.ppt64, 4, a.nx, a.ny, d), a,
                       [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
                         switch (ppt) {
                           case 1: return launch_f64_ppt<M, 1, 4>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
                           case 2: return launch_f64_ppt<M, 2, 3>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
-                          default: return launch_f64_ppt<M, 4, 2>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                          default:
+                            if constexpr (M::kConstRecords) {
+                              if (cb) return launch_f64_const<M>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
+                            }
+                            return launch_f64_ppt<M, 4, 2>(l64, t64, a, out, d, st, tiles_x, b, e, resident);
                         }
                       });
 }
@@ -366,6 +460,30 @@ template <class M>
 int launch_quads(const typename Rec64<M>::type* l64, const LtTables<double>* t64, const GridArgs& a, int quads_per_row,
                  const unsigned int* list, const LtWsHeader* hdr, const unsigned char* flags, double2* out,
                  const DeviceInfo& d, cudaStream_t st) {
+  const long long n_quads_all = (long long)quads_per_row * a.ny;
+  if constexpr (M::kConstRecords) {
+    if (const_records_ok(st, d, out, a.staging, a.n_lens, sizeof(typename Rec64<M>::type))) {
+      int grid_c = 1;
+      const int rc_c = grid_for(lt_grad_quads_f64_const_kernel<M, true>, 0, (n_quads_all + LT_THREADS - 1) / LT_THREADS, d, grid_c);
+      if (rc_c != LT_OK) return rc_c;
+      long long r2 = 0;
+      if (a.staging) {
+        const int rc2 = resident_ctas(lt_grad_quads_f64_const_kernel<M, false>, 0, d, r2);
+        if (rc2 != LT_OK) return rc2;
+      }
+      KernelEvents ke(st);
+      return with_const_records(l64, a.n_lens, d, st, out, a.staging, [&](int cnt, const double2* acc, double2* dst) -> int {
+        if (a.staging)
+          LT_CUDA(launch_dependent(lt_grad_quads_f64_const_kernel<M, false>, grid_c, LT_THREADS, 0, st, t64, cnt, acc, a.x_min,
+                                   a.y_min, a.dx, a.nx, quads_per_row, list, hdr, flags, dst));
+        else
+          LT_CUDA(launch_dependent(lt_grad_quads_f64_const_kernel<M, true>, grid_c, LT_THREADS, 0, st, t64, cnt, acc ? 1 : 0,
+                                   a.x_min, a.y_min, a.dx, a.nx, quads_per_row, list, hdr, flags, dst));
+        ++g_launches;
+        return LT_OK;
+      });
+    }
+  }
   int chunk = 1, grid = 1;
   const int wanted = g_tuning.chunk64;
   int rc = pick_chunk(lt_grad_quads_f64_kernel<M>, a.n_lens, wanted > 0 ? wanted : kDefaultChunk64,
@@ -468,7 +586,7 @@ namespace {
 template <class M>
 int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
                      lt_precision mode, const lt_mixed_params* mixed_or_null, void* d_out_grad, void* d_workspace,
-                     size_t workspace_bytes, void* cuda_stream) {
+                     size_t workspace_bytes, void* cuda_stream, void* d_staging = nullptr) {
   if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
   if (mode != LT_FP64 && mode != LT_FP32 && mode != LT_MIXED) return LT_ERR_BAD_MODE;
   if (!d_out_grad || !d_workspace || (n_lens > 0 && !d_lenses)) return LT_ERR_NULL_POINTER;
@@ -495,7 +613,8 @@ int gradient_grid_impl(const void* d_lenses, int n_lens, double x_min, double y_
   const typename Rec32<M>::type* l32 = reinterpret_cast<const typename Rec32<M>::type*>(ws + L.lens32);
   const LtTables<double>* t64 = reinterpret_cast<const LtTables<double>*>(ws + L.tab64);
   const LtTables<float>* t32 = reinterpret_cast<const LtTables<float>*>(ws + L.tab32);
-  const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
+  GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
+  if (mode != LT_FP32) a.staging = reinterpret_cast<double2*>(d_staging);
 
   if (mode == LT_MIXED)   /* the flag map is cleared before the first kernel so that the kernels follow one another */
     LT_CUDA(cudaMemsetAsync(ws + L.flags, 0, (size_t)n_pix, st));
@@ -628,7 +747,7 @@ int gradient_grid_host_impl(const void* h_lenses, int n_lens, double x_min, doub
       (void)cudaGetLastError();
   }
   const int rc = gradient_grid_impl<M>(d_cat, n_lens, x_min, y_min, dx, nx, ny, mode, mixed_or_null,
-                                       d_direct ? d_direct : d_out, ws, w, st);
+                                       d_direct ? d_direct : d_out, ws, w, st, d_direct ? d_out : nullptr);
   if (rc != LT_OK) return rc;
   if (!d_direct) LT_CUDA(cudaMemcpyAsync(h_out_grad, d_out, (size_t)nx * ny * elem, cudaMemcpyDeviceToHost, st));
   return LT_OK;
@@ -677,6 +796,7 @@ int lt_set_tuning(int ppt64, int ppt32, int chunk64, int chunk32, int ctas_per_s
   g_tuning.points_per_thread = (single_launch >> 2) & 1;
   g_tuning.no_dependent_launch = (single_launch >> 3) & 1;
   g_tuning.plain_sp = (single_launch >> 4) & 1;
+  g_tuning.no_const_records = (single_launch >> 5) & 1;
   g_tuning.ppt64 = ppt64;
   g_tuning.ppt32 = ppt32;
   g_tuning.chunk64 = chunk64;

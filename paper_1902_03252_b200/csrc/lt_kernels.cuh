@@ -171,6 +171,71 @@ lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ le
   }
 }
 
+// ------------------------------------------------------------------------------------------------ fp64 grid kernel, records in the constant bank
+// The same loop with the lens records held in __constant__ memory: a record is read with LDCU.128 into UNIFORM registers
+// (every lane of every warp reads the same record anyway) and the FP64 instructions take those as operands directly,
+// instead of eight broadcast LDS.128 into 32 vector registers per lens.  Same operations in the same order: identical
+// bits; 3.6 % faster (profiles/r02_fp64_pipe_diagnostics.md).  __constant__ memory is per-module state, so the host side
+// (lt_api.cu: ConstSlot) copies at most LT_CONST_SLOT_BYTES of records into the slot per launch, orders the slot's users
+// across streams with an event, and launches once per slot-load: `acc` != null continues the sums that the launch before
+// left there (the partial sum of the lenses so far, exactly the value the one-launch loop carries in registers); `acc` may
+// be `out` itself or a device staging buffer when `out` is pinned host memory (only the last launch writes that).
+// 4 pixels per thread only; the ragged rest of a grid keeps the shared-memory kernels above.
+#define LT_CONST_SLOT_BYTES 57344
+__constant__ double2 lt_const_slot[LT_CONST_SLOT_BYTES / 16];
+
+// INPLACE: `acc` is a flag and the partial sums are read from `out` itself (device output); else `acc` is the buffer they
+// are read from (null: start from zero) -- two instantiations because the in-place form compiles to the faster loop
+template <class M, bool INPLACE>
+__global__ void __launch_bounds__(LT_THREADS, 2)
+lt_grad_f64_const_kernel(const LtTables<double>* __restrict__ tables, int n_lens,
+                         typename LtSelect<INPLACE, int, const double2*>::type acc, double x_min, double y_min, double dx,
+                         int nx, int ny, int tiles_x, int tile_begin, int tile_end, double2* __restrict__ out) {
+  typedef typename M::template Rec<double>::type Rec;
+  __shared__ LtTables<double> tab;
+  lt_grid_dependency_wait();
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  __syncthreads();
+  constexpr int PPT = 4, TILE_W = 32 * PPT;
+  const Rec* cl = reinterpret_cast<const Rec*>(lt_const_slot);
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  for (int tile = tile_begin + blockIdx.x; tile < tile_end; tile += gridDim.x) {
+    const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
+    const int j = ty * LT_TILE_H + wrp;
+    const int i0 = tx * TILE_W + lane;
+    const double t2 = __dadd_rn(y_min, __dmul_rn((double)j, dx));
+    double t1[PPT], G1[PPT], G2[PPT];
+#pragma unroll
+    for (int p = 0; p < PPT; ++p) {
+      const int i = i0 + 32 * p;
+      t1[p] = __dadd_rn(x_min, __dmul_rn((double)i, dx));
+      G1[p] = 0.0;
+      G2[p] = 0.0;
+      if (acc && j < ny && i < nx) {
+        double2 g;
+        if constexpr (INPLACE) g = out[(size_t)j * nx + i];
+        else g = acc[(size_t)j * nx + i];
+        G1[p] = g.x;
+        G2[p] = g.y;
+      }
+    }
+#pragma unroll 1
+    for (int k = 0; k < n_lens; ++k) {
+      const Rec& L = cl[k];
+      const auto row = M::template row_abs<double>(t2, L);
+#pragma unroll
+      for (int p = 0; p < PPT; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
+    }
+    if (j < ny) {
+#pragma unroll
+      for (int p = 0; p < PPT; ++p) {
+        const int i = i0 + 32 * p;
+        if (i < nx) out[(size_t)j * nx + i] = make_double2(G1[p], G2[p]);
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ fp32 grid kernel
 // Same mapping.  Coordinates: for every tile and lens the lens-frame position of the TILE CENTRE
 // is formed in fp64 from the fp64 catalogue while the chunk is staged (a few fp64 operations per lens per tile, i.e.
@@ -485,6 +550,57 @@ lt_grad_quads_f64_kernel(const typename M::template Rec<double>::type* __restric
 #pragma unroll
         for (int p = 0; p < 4; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
       }
+    }
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+      if (keep[p]) out[p0 + p] = make_double2(G1[p], G2[p]);
+  }
+}
+
+// the quad kernel with the records in the constant bank (see lt_grad_f64_const_kernel): `acc` != null continues the
+// sums of the flagged pixels that the launch before stored there
+template <class M, bool INPLACE>
+__global__ void __launch_bounds__(LT_THREADS, 2)
+lt_grad_quads_f64_const_kernel(const LtTables<double>* __restrict__ tables, int n_lens,
+                               typename LtSelect<INPLACE, int, const double2*>::type acc, double x_min, double y_min, double dx,
+                               int nx, int quads_per_row, const unsigned int* __restrict__ list,
+                               const LtWsHeader* __restrict__ hdr, const unsigned char* __restrict__ flags,
+                               double2* __restrict__ out) {
+  typedef typename M::template Rec<double>::type Rec;
+  __shared__ LtTables<double> tab;
+  lt_grid_dependency_wait();
+  if (M::kTables) lt_copy16(&tab, tables, (int)(sizeof(tab) / 16));
+  __syncthreads();
+  const Rec* cl = reinterpret_cast<const Rec*>(lt_const_slot);
+  const long long total = (long long)hdr->list_count;
+  for (long long g = (long long)blockIdx.x * LT_THREADS + threadIdx.x; g < total; g += (long long)gridDim.x * LT_THREADS) {
+    const unsigned int q = list[g];
+    const int j = (int)(q / (unsigned int)quads_per_row);
+    const int i0 = (int)(q - (unsigned int)j * (unsigned int)quads_per_row) * 4;
+    const size_t p0 = (size_t)j * nx + (size_t)i0;
+    const double t2 = __dadd_rn(y_min, __dmul_rn((double)j, dx));
+    double t1[4], G1[4], G2[4];
+    bool keep[4];
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      t1[p] = __dadd_rn(x_min, __dmul_rn((double)(i0 + p), dx));
+      G1[p] = 0.0;
+      G2[p] = 0.0;
+      keep[p] = i0 + p < nx && flags[p0 + p] != 0;
+      if (acc && keep[p]) {
+        double2 v;
+        if constexpr (INPLACE) v = out[p0 + p];
+        else v = acc[p0 + p];
+        G1[p] = v.x;
+        G2[p] = v.y;
+      }
+    }
+#pragma unroll 1
+    for (int k = 0; k < n_lens; ++k) {
+      const Rec& L = cl[k];
+      const auto row = M::template row_abs<double>(t2, L);
+#pragma unroll
+      for (int p = 0; p < 4; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
     }
 #pragma unroll
     for (int p = 0; p < 4; ++p)

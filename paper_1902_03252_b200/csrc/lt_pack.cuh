@@ -158,6 +158,7 @@ struct LtDpieModel {
   static constexpr bool kTables = true;
   static constexpr bool kSkyFrame32 = false;
   static constexpr bool kPacked32 = true;      // the fp32 grid kernel evaluates two pixels per instruction (interact_lens_x2)
+  static constexpr bool kConstRecords = true;  // fp64 kernels: records from the constant bank where the call allows it (+3 % at config 3)
 #if defined(__CUDACC__)
   static __device__ __forceinline__ void interact_lens_x2(const lt_f2 X, const lt_f2 Y, const LtLens<float>& L,
                                                           const LtTables2& tab, lt_f2& G1, lt_f2& G2) {
@@ -201,6 +202,7 @@ struct LtSieModel {
   static constexpr bool kTables = false;
   static constexpr bool kSkyFrame32 = true;
   static constexpr bool kPacked32 = true;
+  static constexpr bool kConstRecords = false; // measured: 48-byte records, 3 LDS.128 against 5 LDCU per lens: 3.7 % slower
 #if defined(__CUDACC__)
   static __device__ __forceinline__ void interact_sky_x2(const lt_f2 d1, const LtSieRow<float>& r, const LtSieLens<float>& L,
                                                          const LtTables2&, lt_f2& G1, lt_f2& G2) {
@@ -234,6 +236,7 @@ struct LtNfwModel {
   static constexpr bool kTables = true;
   static constexpr bool kSkyFrame32 = true;
   static constexpr bool kPacked32 = false;
+  static constexpr bool kConstRecords = false;
   static LT_HD bool valid(const Raw& r) { return lt_nfw_valid(r); }
   static LT_HD void pack(const Raw& r, LtNfwLens<double>& L) { lt_pack_nfw(r, L); }
   static LT_HD void poison(LtNfwLens<double>& L) { lt_poison_nfw(L); }

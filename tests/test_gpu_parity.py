@@ -93,6 +93,48 @@ def test_launch_configurations_agree(env, ppt64, ppt32, chunk):
     assert _err(a, ref) < TOL_F64 and _err(b, ref) < TOL_F32
 
 
+@pytest.mark.parametrize("n_lens,nx,ny", [(100, 1500, 700), (449, 1300, 333), (1000, 1111, 600)])
+def test_records_from_the_constant_bank_give_the_same_bits(env, n_lens, nx, ny):
+    """The fp64 kernels read the lens records from __constant__ memory where the call allows it (one slot of 448 dPIE
+    records: 449 and 1000 lenses take two and three launches that continue each other's sums); lt_set_tuning bit 5 keeps
+    them in shared memory.  Same operations in the same order: fp64 and mixed maps bit-equal, on grids with whole waves
+    and a ragged rest, also when two streams use the slot alternately."""
+    torch, lt, O = env
+    L = workloads.random_catalogue(31 + n_lens, n_lens, L=60.0)
+    W = workloads.Workload("const", L, -60.0, -25.0, 0.085, nx, ny, 0)
+    res = {}
+    for bit in (0, 32):
+        try:
+            lt.lt_set_tuning(single_launch=bit)
+            res[bit] = (_gpu_map(torch, lt, W, lt.LT_FP64), _gpu_map(torch, lt, W, lt.LT_MIXED))
+        finally:
+            lt.lt_set_tuning()
+    assert np.array_equal(res[0][0], res[32][0]) and np.array_equal(res[0][1], res[32][1])
+    assert lt.lt_last_launch_count() >= 1
+    # two streams, two different catalogues, interleaved calls: each map equals its single-stream result
+    L2 = workloads.random_catalogue(77, n_lens, L=60.0)
+    d1, d2 = torch.from_numpy(L).cuda(), torch.from_numpy(L2).cuda()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    ref2 = lt.lt_gradient_grid(d2, W.x_min, W.y_min, W.dx, nx, ny, lt.LT_FP64).cpu().numpy()
+    outs = []
+    for rep in range(3):
+        a = lt.lt_gradient_grid(d1, W.x_min, W.y_min, W.dx, nx, ny, lt.LT_FP64, stream=s1)
+        b = lt.lt_gradient_grid(d2, W.x_min, W.y_min, W.dx, nx, ny, lt.LT_FP64, stream=s2)
+        outs.append((a, b))
+    torch.cuda.synchronize()
+    for a, b in outs:
+        assert np.array_equal(a.cpu().numpy(), res[0][0]) and np.array_equal(b.cpu().numpy(), ref2)
+    # the host entry point: the map goes straight into pinned host memory; with several slot-loads the partial sums stay in
+    # the call's device staging buffer and only the last launch writes across PCIe
+    hL = torch.from_numpy(L).pin_memory()
+    for mode, k in ((lt.LT_FP64, 0), (lt.LT_MIXED, 1)):
+        hout = torch.full((ny, nx, 2), float("nan"), dtype=torch.float64).pin_memory()
+        wsh = lt.alloc_workspace(n_lens, nx, ny, mode, host=True)
+        lt.lt_gradient_grid_host(hL, W.x_min, W.y_min, W.dx, nx, ny, mode, hout, wsh)
+        torch.cuda.synchronize()
+        assert np.array_equal(hout.numpy(), res[0][k])
+
+
 def test_oversized_chunk_request_is_clamped(env):
     """lt_set_tuning(chunk64 = chunk32 = 65536) with 4096 lenses: the wanted chunk exceeds what fits beside each kernel's
     own static shared memory (the range-reduction tables) under the opt-in limit; the library clamps it per kernel instead
