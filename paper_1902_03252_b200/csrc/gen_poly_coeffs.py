@@ -2,6 +2,9 @@
 
 Near-minimax by interpolation at Chebyshev nodes in t = z^2 (mpmath, 50 digits), converted to the monomial basis;
 prints C arrays and the measured max relative error of the fp64-rounded (resp. fp32-rounded) polynomial.
+The fp64 arrays the kernels use are the `_HI` ones: the leading coefficient is rounded to a double whose low 32 bits are
+zero (it is then an immediate of the first FMA of the Horner chain, which so reads one constant register instead of two:
+lt_math.cuh) and the lower coefficients are refitted around it with the constant term exactly 1.
 CUDA-path only: the CPU oracle uses libm/libquadmath log and atan2 and shares nothing with this.
 
     python paper_1902_03252_b200/csrc/gen_poly_coeffs.py
@@ -50,6 +53,39 @@ def max_err(g, tmax, coeffs, rnd):
     return worst
 
 
+def hi_only(x):
+    """nearest double whose low word is zero (21 significant bits): encodable as an FP64 immediate"""
+    import struct
+    b = struct.unpack('<Q', struct.pack('<d', float(x)))[0]
+    lo = b & 0xffffffff
+    b = (b & ~0xffffffff) + (0x100000000 if lo >= 0x80000000 else 0)
+    return struct.unpack('<d', struct.pack('<Q', b))[0]
+
+
+def refit_below(g, tmax, n, top):
+    """degree n with c0 = 1 and c_n = top fixed: (g - 1 - top t^n) / t interpolated at n - 1 Chebyshev nodes"""
+    m = n - 1
+    nodes = [tmax * (1 + mp.cos(mp.pi * (2 * k + 1) / (2 * m))) / 2 for k in range(m)]
+    A = mp.matrix(m, m)
+    b = mp.matrix(m, 1)
+    for i, t in enumerate(nodes):
+        for j in range(m):
+            A[i, j] = t ** j
+        b[i] = (g(t) - 1 - mp.mpf(top) * t ** n) / t
+    c = mp.lu_solve(A, b)
+    return [mp.mpf(1)] + [c[j] for j in range(m)] + [mp.mpf(top)]
+
+
+def emit_hi(name, g, zmax, n):
+    tmax = mp.mpf(zmax) ** 2
+    top = hi_only(cheb_fit(g, tmax, n)[n])
+    c = refit_below(g, tmax, n, top)
+    err = max_err(g, tmax, c, float)
+    print("// %s: degree %d in t=z^2, |z| <= %s, leading coefficient %s (low word zero), max rel err %s"
+          % (name, n, mp.nstr(mp.mpf(zmax), 8), float(top).hex(), mp.nstr(err, 3)))
+    print("static const double %s[%d] = {%s};" % (name, n + 1, ", ".join("%.17e" % float(x) for x in c)))
+
+
 def f32(c):
     import numpy as np
     return float(np.float32(float(c)))
@@ -74,6 +110,8 @@ if __name__ == "__main__":
         emit("LT_ATAN_P64_%d" % n, g_atan, zr, n, float, "")
     for n in (3, 4, 5):
         emit("LT_ATANH_P64_%d" % n, g_atanh, zr, n, float, "")
+    emit_hi("LT_ATAN_P64_4_HI", g_atan, zr, 4)
+    emit_hi("LT_ATANH_P64_4_HI", g_atanh, zr, 4)
     for n in (1, 2, 3):
         emit("LT_ATAN_P32_%d" % n, g_atan, zr, n, f32, "f")
     for n in (1, 2, 3):

@@ -40,7 +40,7 @@ LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
   L.x0 = r.x;
   L.y0 = r.y;
   L.Kc = (ome * r.rcore * rf) * (ome * r.rcore * rf);  // q^2 s_c^2 / f^2
-  L.Kt = (ome * r.rcut * rf) * (ome * r.rcut * rf);
+  L.dK = (ome * rf) * (ome * rf) * ((r.rcut - r.rcore) * (r.rcut + r.rcore));   // K_t - K_c without cancellation
   L.sc = sc * rf;
   L.st = st * rf;
   L.q2sc = q2 * sc * rf;
@@ -54,7 +54,7 @@ LT_HD void lt_pack_lens(const LtRawLens& r, LtLens<double>& L) {
 
 LT_HD void lt_poison_lens(LtLens<double>& L) {  // invalid parameters: the lens contributes NaN everywhere
   const double n = NAN;
-  L.x0 = L.y0 = L.cx = L.sx = L.cy = L.sy = L.Kc = L.Kt = L.sc = L.st = L.q2sc = L.q2st = L.g = L.f = L.Cc = L.Cs = n;
+  L.x0 = L.y0 = L.cx = L.sx = L.cy = L.sy = L.Kc = L.dK = L.sc = L.st = L.q2sc = L.q2st = L.g = L.f = L.Cc = L.Cs = n;
 }
 
 // fp32 record = fp64 record rounded once, except x0, y0 which the fp32 kernel fills per pixel tile (lens-frame
@@ -67,7 +67,7 @@ LT_HD void lt_round_lens(const LtLens<double>& D, double dx, LtLens<float>& F) {
   F.cy = (float)(dx * D.cy);
   F.sy = (float)(dx * D.sy);
   F.Kc = (float)D.Kc;
-  F.Kt = (float)D.Kt;
+  F.dK = (float)D.dK;
   F.sc = (float)D.sc;
   F.st = (float)D.st;
   F.q2sc = (float)D.q2sc;
