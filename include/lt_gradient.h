@@ -76,7 +76,8 @@ typedef enum {
   LT_ERR_MISALIGNED = -6,      /* d_out_grad or d_workspace not 16-byte aligned                                  */
   LT_ERR_BAD_MIXED_PARAMS = -7,
   LT_ERR_CUDA = -8,            /* a launch or runtime call failed; lt_last_cuda_error() has the cudaError_t      */
-  LT_ERR_BAD_LENS_PARAMS = -9  /* reported by lt_last_status only (device-side domain check)                     */
+  LT_ERR_BAD_LENS_PARAMS = -9, /* reported by lt_last_status only (device-side domain check)                     */
+  LT_ERR_NOALLOC_TOO_LARGE = -10 /* lt_gradient_grid_noalloc: n_lens > LT_NOALLOC_MAX_LENSES                       */
 } lt_status;
 
 typedef struct {               /* mixed-rule constants; lt_mixed_defaults() gives the paper's values             */
@@ -342,6 +343,33 @@ int lt_rule_audit(const float* d_sp_map, const double* d_dp_map, double x_min, d
 /* Copies the result of lt_rule_audit to the host (synchronises cuda_stream) and fills the two implied_m_max fields
  * (M_max = (dx / 4) / E_SP; inf when the error is 0). */
 int lt_rule_audit_result(const lt_audit_result* d_result, double dx, void* cuda_stream, lt_audit_result* h_out);
+
+/* lt_gradient_grid without any allocation, by the library or by the caller: the deflection map of dPIE lenses (the same
+ * operation as lt_gradient_grid: Algorithm 1, with the dPIE body of BASELINE.json's north star) for
+ * mode = LT_FP64 or LT_FP32, with the workspace -- the scratch that the per-lens precompute kernel writes and the grid
+ * kernels read -- held in a device array built into the library (LT_NOALLOC_SCRATCH_BYTES = 800 KiB of device memory on
+ * every GPU that loads the library, until the process exits).  For callers that cannot call cudaMalloc: code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it.  The call itself makes no cudaMalloc / cudaFree and calls
+ * no allocating library routine; it enqueues the precompute kernel and the shared-memory grid kernels on cuda_stream and
+ * returns (asynchronous, like lt_gradient_grid).
+ *   d_lenses   device, [n_lens] lt_lens, caller-owned, read only; 0 <= n_lens <= LT_NOALLOC_MAX_LENSES (4096).
+ *   d_out_grad device, [ny][nx][2] double (LT_FP64) or float (LT_FP32), 16-byte aligned, caller-owned, every element
+ *              written.  Grid arguments as for lt_gradient_grid.
+ * Results: LT_FP32 bit-identical to lt_gradient_grid; LT_FP64 the same operations in the same order as lt_gradient_grid
+ * (identical bits; the records come from shared memory instead of the constant bank).
+ * Sharing: every call on a device uses the SAME array.  It keeps the last call's contents; nothing in it has to start at
+ * zero (the precompute kernel rewrites the header, the domain-check slots, the tables and every record the call reads).
+ * Two calls that overlap on the GPU (different streams, or different host threads) RACE on it: order them on one stream
+ * or with events.  lt_noalloc_last_status reports the domain check of the LAST call on the current device.
+ * Errors: LT_ERR_NOALLOC_TOO_LARGE (n_lens > LT_NOALLOC_MAX_LENSES: use lt_gradient_grid with a workspace),
+ * LT_ERR_BAD_MODE (LT_MIXED: its scratch grows with the map), LT_ERR_BAD_SIZE, LT_ERR_NULL_POINTER, LT_ERR_BAD_GRID,
+ * LT_ERR_MISALIGNED, LT_ERR_CUDA -- all argument errors before any CUDA call. */
+#define LT_NOALLOC_MAX_LENSES 4096
+#define LT_NOALLOC_SCRATCH_BYTES 819200
+int lt_gradient_grid_noalloc(const lt_lens* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                             lt_precision mode, void* d_out_grad, void* cuda_stream);
+/* lt_last_status for the built-in scratch of the current device (synchronises cuda_stream). */
+int lt_noalloc_last_status(void* cuda_stream, int* bad_lens_or_null);
 
 /* FMA-chain microbenchmarks used by bench.py to confirm the FP64 / FP32 peaks on the device in the same run
  * (SURVEY 8(d)): runs `iters` dependent-free FMAs per thread on a full grid; returns achieved FLOP/s in *flops_out

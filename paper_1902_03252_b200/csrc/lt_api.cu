@@ -772,6 +772,7 @@ const char* lt_error_string(int code) {
     case LT_ERR_BAD_MIXED_PARAMS: return "bad mixed-rule parameters";
     case LT_ERR_CUDA: return "CUDA runtime error (see lt_last_cuda_error)";
     case LT_ERR_BAD_LENS_PARAMS: return "lens parameters outside the domain (e in [0,1), 0 < rcore < rcut, finite)";
+    case LT_ERR_NOALLOC_TOO_LARGE: return "catalogue larger than the built-in scratch of lt_gradient_grid_noalloc (LT_NOALLOC_MAX_LENSES)";
   }
   return "unknown error code";
 }
@@ -1086,6 +1087,85 @@ int lt_rule_audit_result(const lt_audit_result* d_result, double dx, void* cuda_
   h_out->implied_m_max = dx / 4.0 / h_out->max_err;                                /* P:284 */
   h_out->implied_m_max_outside_patch = dx / 4.0 / h_out->max_err_outside_patch;
   return LT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ no-allocation entry point
+// For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+// forbid cudaMalloc): lt_gradient_grid for LT_FP64 / LT_FP32 with the workspace -- the scratch the precompute kernel
+// writes (header, domain-check slots, range-reduction tables, packed fp64 / fp32 records) and the grid kernels read --
+// in a file-scope device array instead of a caller-allocated buffer.  LT_NOALLOC_SCRATCH_BYTES (800 KiB) per GPU that
+// loads the library, held until exit.  In host code `lt_noalloc_scratch` is a host-side stand-in, not a device address:
+// its device address is taken once per device with cudaGetSymbolAddress (that device current) and passed to the kernels.
+static __device__ __align__(256) unsigned char lt_noalloc_scratch[LT_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+std::mutex g_noalloc_mu;
+void* g_noalloc_ptr[64] = {};
+
+// device address of the scratch array on the current device (set up on first use, per device)
+int noalloc_scratch(const DeviceInfo& d, unsigned char** out) {
+  if (d.device < 0 || d.device >= 64) return LT_ERR_BAD_SIZE;
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[d.device]) {
+    void* p = nullptr;
+    LT_CUDA(cudaGetSymbolAddress(&p, lt_noalloc_scratch));
+    if (!p) return cuda_fail(cudaErrorInvalidSymbol);
+    g_noalloc_ptr[d.device] = p;
+  }
+  *out = (unsigned char*)g_noalloc_ptr[d.device];
+  return LT_OK;
+}
+}  // namespace
+
+int lt_gradient_grid_noalloc(const lt_lens* d_lenses, int n_lens, double x_min, double y_min, double dx, int nx, int ny,
+                             lt_precision mode, void* d_out_grad, void* cuda_stream) {
+  typedef LtDpieModel M;
+  if (!sizes_ok(n_lens, nx, ny)) return LT_ERR_BAD_SIZE;
+  if (mode != LT_FP64 && mode != LT_FP32) return LT_ERR_BAD_MODE;      /* mixed scratch grows with the map: not here */
+  if (n_lens > LT_NOALLOC_MAX_LENSES) return LT_ERR_NOALLOC_TOO_LARGE;
+  if (!d_out_grad || (n_lens > 0 && !d_lenses)) return LT_ERR_NULL_POINTER;
+  if (!(isfinite(x_min) && isfinite(y_min) && isfinite(dx)) || !(dx > 0.0)) return LT_ERR_BAD_GRID;
+  if ((uintptr_t)d_out_grad & 15) return LT_ERR_MISALIGNED;
+  const Layout L = make_layout(n_lens, (long long)nx * ny, false);
+  if (L.total > (size_t)LT_NOALLOC_SCRATCH_BYTES) return LT_ERR_NOALLOC_TOO_LARGE;
+  DeviceInfo dev;
+  int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  unsigned char* ws = nullptr;
+  rc = noalloc_scratch(dev, &ws);
+  if (rc != LT_OK) return rc;
+  g_launches = 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const Rec64<M>::type* l64 = reinterpret_cast<const Rec64<M>::type*>(ws + L.lens64);
+  const Rec32<M>::type* l32 = reinterpret_cast<const Rec32<M>::type*>(ws + L.lens32);
+  const LtTables<double>* t64 = reinterpret_cast<const LtTables<double>*>(ws + L.tab64);
+  const LtTables<float>* t32 = reinterpret_cast<const LtTables<float>*>(ws + L.tab32);
+  const GridArgs a{n_lens, x_min, y_min, dx, nx, ny};
+  /* Nothing of the last call's contents is read before it is rewritten: the precompute kernel initialises the header and
+   * the domain-check slots of this call with plain stores and writes every record and table entry the grid kernels read. */
+  rc = precompute<M>(d_lenses, n_lens, dx, ws, L, st);                                       /* a1 */
+  if (rc != LT_OK) return rc;
+  if (mode == LT_FP32) return launch_f32<M>(l64, l32, t32, a, (float2*)d_out_grad, dev, st, /*hook=*/false);
+  /* fp64: the shared-memory grid kernels at every pixels-per-thread (the constant-bank variant of lt_gradient_grid
+   * creates an event on its first use; same operations in the same order, identical bits) */
+  return launch_waves(pick_ppt(g_tuning.ppt64, 4, a.nx, a.ny, dev), a,
+                      [&](int ppt, int tiles_x, long long b, long long e, long long* resident) {
+                        switch (ppt) {
+                          case 1: return launch_f64_ppt<M, 1, 4>(l64, t64, a, (double2*)d_out_grad, dev, st, tiles_x, b, e, resident);
+                          case 2: return launch_f64_ppt<M, 2, 3>(l64, t64, a, (double2*)d_out_grad, dev, st, tiles_x, b, e, resident);
+                          default: return launch_f64_ppt<M, 4, 2>(l64, t64, a, (double2*)d_out_grad, dev, st, tiles_x, b, e, resident);
+                        }
+                      });
+}
+
+int lt_noalloc_last_status(void* cuda_stream, int* bad_lens_or_null) {
+  DeviceInfo dev;
+  int rc = device_info(dev);
+  if (rc != LT_OK) return rc;
+  unsigned char* ws = nullptr;
+  rc = noalloc_scratch(dev, &ws);
+  if (rc != LT_OK) return rc;
+  return lt_last_status(ws, cuda_stream, bad_lens_or_null);
 }
 
 int lt_peak_probe(int which, int iters, double* flops_out, void* cuda_stream) {

@@ -25,7 +25,10 @@ SYMBOLS = ["lt_version", "lt_error_string", "lt_last_cuda_error", "lt_mixed_defa
            "lt_gradient_grid_sie", "lt_gradient_points_sie", "lt_gradient_grid_sie_host", "lt_find_images", "lt_mixed_rule",
            "lt_source_barycentres", "lt_chi2",
            "lt_gradient_grid_nfw", "lt_gradient_points_nfw", "lt_gradient_grid_nfw_host",
-           "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_mixed_last_sp_map", "lt_rule_audit", "lt_rule_audit_result", "lt_peak_probe"]
+           "lt_set_tuning", "lt_last_launch_count", "lt_set_kernel_events", "lt_last_status", "lt_mixed_last_stats", "lt_mixed_last_flags", "lt_mixed_last_sp_map", "lt_rule_audit", "lt_rule_audit_result", "lt_peak_probe",
+           "lt_gradient_grid_noalloc", "lt_noalloc_last_status"]
+LT_NOALLOC_MAX_LENSES = 4096
+LT_ERR_NOALLOC_TOO_LARGE = -10
 
 
 class lt_mixed_params(ctypes.Structure):
@@ -120,6 +123,10 @@ def lib():
         L.lt_rule_audit_result.restype = ci
         L.lt_peak_probe.argtypes = [ci, ci, ctypes.POINTER(cd), vp]
         L.lt_peak_probe.restype = ci
+        L.lt_gradient_grid_noalloc.argtypes = [vp, ci, cd, cd, cd, ci, ci, ci, vp, vp]
+        L.lt_gradient_grid_noalloc.restype = ci
+        L.lt_noalloc_last_status.argtypes = [vp, ctypes.POINTER(ci)]
+        L.lt_noalloc_last_status.restype = ci
         _lib = L
     return _lib
 
@@ -226,6 +233,32 @@ def lt_gradient_grid(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None,
     _check(rc, _fn)
     _keep(stream, lenses, workspace, out)
     return out
+
+
+def lt_gradient_grid_noalloc(lenses, x_min, y_min, dx, nx, ny, mode, out, stream=None):
+    """lt_gradient_grid (LT_FP64 / LT_FP32, at most LT_NOALLOC_MAX_LENSES dPIE lenses) with the workspace in the library's
+    built-in device array: neither this binding nor the library allocates.  `lenses` (CUDA float64 [n_lens, 7], contiguous)
+    and `out` ([ny, nx, 2], float64 / float32) are the caller's.  Calls that overlap on the GPU race on the array."""
+    if not (lenses.is_cuda and lenses.dtype == torch.float64 and lenses.is_contiguous() and lenses.dim() == 2 and
+            lenses.shape[1] == 7):
+        raise TypeError("lenses must be a contiguous CUDA float64 [n_lens, 7] tensor")
+    dt = torch.float32 if mode == LT_FP32 else torch.float64
+    if out.dtype != dt or out.numel() != nx * ny * 2 or not out.is_contiguous() or not out.is_cuda:
+        raise TypeError("out must be a contiguous CUDA %s tensor with nx*ny*2 elements" % dt)
+    n_lens = lenses.shape[0]
+    _check(lib().lt_gradient_grid_noalloc(ctypes.c_void_p(lenses.data_ptr() if n_lens else None), n_lens, float(x_min),
+                                          float(y_min), float(dx), int(nx), int(ny), int(mode),
+                                          ctypes.c_void_p(out.data_ptr()), _stream(stream)), "lt_gradient_grid_noalloc")
+    return out
+
+
+def lt_noalloc_last_status(stream=None):
+    """(code, first offending lens index or -1) of the last lt_gradient_grid_noalloc call on the current device."""
+    bad = ctypes.c_int(-1)
+    rc = lib().lt_noalloc_last_status(_stream(stream), ctypes.byref(bad))
+    if rc not in (LT_OK, LT_ERR_BAD_LENS_PARAMS):
+        raise LtError(rc, "lt_noalloc_last_status")
+    return rc, bad.value
 
 
 def lt_gradient_grid_sie(lenses, x_min, y_min, dx, nx, ny, mode=LT_FP64, mixed=None, out=None, workspace=None,

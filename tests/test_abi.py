@@ -42,7 +42,7 @@ def test_host_only_entry_points(L):
     assert (p.m_max, p.patch_halfwidth_cluster, p.patch_halfwidth_galaxy, p.b0_cluster_threshold) == (3.26, 6.0, 0.3, 15.0)
     assert abs(p.c28 * 0.03 - 0.0104) < 1e-15                      # eq. 28 at the paper's 0.03"/px
     assert round(0.03 / p.m_max, 4) == 0.0092                      # eq. 25
-    for code in range(-9, 1):
+    for code in range(-10, 1):
         assert L.lib().lt_error_string(code) not in (None, b"unknown error code")
     assert L.lib().lt_error_string(-99) == b"unknown error code"
 
@@ -75,6 +75,8 @@ def test_argument_errors_need_no_gpu(L):
     bad = L.lt_mixed_params(-1.0, 0.3, 6.0, 0.3, 15.0)
     assert lib.lt_gradient_grid(vp(16), 4, 0.0, 0.0, 1.0, 8, 8, 2, ctypes.byref(bad), vp(16), vp(16), 1 << 20, None) == -7
     assert lib.lt_gradient_points(vp(16), 4, vp(16), -1, vp(16), vp(16), 1 << 20, None) == -2
+    assert lib.lt_gradient_grid_noalloc(vp(16), 4097, 0.0, 0.0, 1.0, 8, 8, 0, vp(16), None) == -10   # LT_NOALLOC_MAX_LENSES
+    assert lib.lt_gradient_grid_noalloc(vp(16), 4, 0.0, 0.0, 1.0, 8, 8, 2, vp(16), None) == -4
     assert lib.lt_set_tuning(-1, 0, 0, 0, 0, 0) == -2 and lib.lt_set_tuning(0, 0, 0, 0, 0, 0) == 0
     assert lib.lt_source_barycentres(vp(16), vp(16), vp(16), -1, 1.0, vp(16), None) == -2
     assert lib.lt_source_barycentres(vp(16), None, vp(16), 3, 1.0, vp(16), None) == -1
