@@ -60,16 +60,30 @@ F_NOM = {"dpie": 69.0,
 PAPER_V100_SIE = {"fp64": 6.9e10, "mixed": 8.2e10}
 # lanes per SM behind the "alu" peaks (paper's Table 1 convention: 2 ops/cycle x clock x lanes)
 LANES = {"fp64": 64, "fp32": 128, "mixed": 64}
-KERNEL_NAME = {"fp64": "lt_grad_f64_kernel", "fp32": "lt_grad_f32_kernel", "mixed": "lt_grad_list_f64_kernel"}
+MODEL_TYPE = {"dpie": "LtDpieModel", "sie": "LtSieModel", "nfw": "LtNfwModel"}
+
+
+def kernel_name(model, mode):
+    """The dominant kernel of a step (the 4-pixel launch; the dPIE fp64 kernels read their records from the constant bank)."""
+    const = "_const" if model == "dpie" else ""
+    return {"fp64": "lt_grad_f64%s_kernel<%s>" % (const, MODEL_TYPE[model]),
+            "fp32": "lt_grad_f32_kernel<%s, 4, 3>" % MODEL_TYPE[model],
+            "mixed": "lt_grad_quads_f64%s_kernel<%s>" % (const, MODEL_TYPE[model])}[mode]
+
+
+
 # Cycles per interaction that the inner loops of the library as built at HEAD need on the pipe that bounds them, from
 # the SASS (cuobjdump -sass; profiles/README.md says how): (pipe, instructions of that pipe per interaction, cycles each
-# holds the SMSP's pipe for one warp).  fp64 / mixed: FP64 instructions, 16 lanes, 2 cycles; fp32: the FMA pipe takes a
-# packed FFMA2 / FMUL2 / FADD2 for 2 cycles (32 lanes, two results each); SIE fp32: one MUFU.RSQ per interaction on the
-# 4-lane XU, 8 cycles -- above its 7.75 FMA-pipe cycles.
-PIPE_FLOOR = {("dpie", "fp64"): ("fp64", 61.75, 2.0), ("dpie", "mixed"): ("fp64", 61.75, 2.0),
-              ("dpie", "fp32"): ("fp32 fma (packed pairs)", 20.25, 2.0),
-              ("sie", "fp64"): ("fp64", 12.75, 2.0), ("sie", "mixed"): ("fp64", 12.75, 2.0),
-              ("sie", "fp32"): ("xu (MUFU.RSQ)", 1.0, 8.0)}
+# holds the SMSP's pipe for one warp, cycles per interaction with the register-file read rate counted).  fp64 / mixed: FP64
+# instructions, 16 lanes, 2 cycles; fp32: the FMA pipe takes a packed FFMA2 / FMUL2 / FADD2 for 2 cycles (32 lanes, two
+# results each); SIE fp32: one MUFU.RSQ per interaction on the 4-lane XU, 8 cycles.  Fourth entry: an FP64 or packed FP32
+# instruction whose sources are THREE distinct register pairs holds the pipe for 3 cycles, not 2 (the register file
+# delivers two 32-bit source reads per lane and cycle: lt_peak_probe 3 / 4, `peak_probe` below; DESIGN.md section 8) --
+# per interaction max(2, source words / 2) summed over the loop's pipe instructions.
+PIPE_FLOOR = {("dpie", "fp64"): ("fp64", 60.75, 2.0, 128.5), ("dpie", "mixed"): ("fp64", 60.75, 2.0, 128.5),
+              ("dpie", "fp32"): ("fp32 fma (packed pairs)", 20.0, 2.0, 44.5),
+              ("sie", "fp64"): ("fp64", 12.75, 2.0, 30.5), ("sie", "mixed"): ("fp64", 12.75, 2.0, 30.5),
+              ("sie", "fp32"): ("xu (MUFU.RSQ)", 1.0, 8.0, 9.25)}
 # dram__bytes_{read,write}.sum per launch of the dominant kernels, written by the ncu recipe of profiles/README.md
 NCU_TRAFFIC_JSON = os.path.join(ROOT, "profiles", "ncu_traffic.json")
 MIXED_SIE = (3.26, 0.0104 / 0.03, 6.0, 0.3, 1.0)   # the paper's rule at its own pixel size; cluster-scale = b0 >= 1"
@@ -462,10 +476,13 @@ class Bench:
         entry = PIPE_FLOOR.get((model, mode))
         if entry is None:
             return None
-        pipe, per, cyc = entry
+        pipe, per, cyc, rf_cyc = entry
         floor = self.sms * 4 * self.sm_max * 1e6 * 32 / (per * cyc)     # interactions per second at 100 % of the pipe
+        rf_floor = self.sms * 4 * self.sm_max * 1e6 * 32 / rf_cyc       # ... with three-register-source instructions at 3 cycles
         return {"pipe": pipe, "instructions_per_interaction": per, "cycles_per_instruction": cyc,
-                "floor_interactions_per_s": floor, "frac_of_floor": units / (ms_k * 1e-3) / floor}
+                "floor_interactions_per_s": floor, "frac_of_floor": units / (ms_k * 1e-3) / floor,
+                "cycles_per_interaction_with_register_reads": rf_cyc,
+                "frac_of_register_read_floor": units / (ms_k * 1e-3) / rf_floor}
 
     def roofline(self, W, m, mode):
         r = m["runner"]
@@ -475,7 +492,7 @@ class Bench:
         peak = 2.0 * self.sms * LANES[mode] * self.sm_max * 1e6 / 1e12
         ach = r.f_nom * units / (ms_k * 1e-3) / 1e12
         tr = ncu_traffic(W.name, mode)
-        return {"bound": "alu", "kernel": KERNEL_NAME[mode], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+        return {"bound": "alu", "kernel": kernel_name(r.model, mode), "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": ach / peak, "frac_at_sampled_clock": ach / (peak * self.sm_run / self.sm_max),
                 "traffic": tr["bytes"] if tr else None, "traffic_source": tr,
                 "peak_source": "derived: 2 x %d SMs x %d lanes x %.0f MHz (DESIGN.md section 8); no FP%s vector peak in "
@@ -765,7 +782,10 @@ def run_ours(args, W):
             p64, p32 = lt.lt_peak_probe(0, 1 << 15), lt.lt_peak_probe(1, 1 << 16)
             line["peak_probe"] = {"fp64_tflops": p64 / 1e12, "fp32_tflops": p32 / 1e12,
                                   "fp32_packed_ffma2_tflops": lt.lt_peak_probe(2, 1 << 15) / 1e12,
-                                  "how": "dependent-free FMA chains, full grid, same process"}
+                                  "fp64_three_register_sources_tflops": lt.lt_peak_probe(3, 1 << 14) / 1e12,
+                                  "fp32_packed_three_register_sources_tflops": lt.lt_peak_probe(4, 1 << 14) / 1e12,
+                                  "how": "dependent-free FMA chains, full grid, same process; the last two with "
+                                         "three distinct register-pair sources per instruction (2/3 of the rate)"}
             line["roofline"]["frac_of_probe"] = line["roofline"]["achieved"] / (
                 (p64 if LANES[args.mode] == 64 else p32) / 1e12)
 

@@ -519,7 +519,8 @@ def lt_rule_audit_result(d_result, dx, stream=None):
 
 
 def lt_peak_probe(which, iters=1 << 16, stream=None):
-    """Achieved FLOP/s of a dependent-free FMA-chain kernel (0 = fp64, 1 = fp32, 2 = fp32 packed pairs).  Synchronises."""
+    """Achieved FLOP/s of a dependent-free FMA-chain kernel (0 = fp64, 1 = fp32, 2 = fp32 packed pairs; 3 = fp64 and
+    4 = packed fp32 with three distinct register sources per instruction).  Synchronises."""
     v = ctypes.c_double(0.0)
     _check(lib().lt_peak_probe(int(which), int(iters), ctypes.byref(v), _stream(stream)), "lt_peak_probe")
     return v.value
