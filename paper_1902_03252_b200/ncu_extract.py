@@ -75,6 +75,9 @@ def main():
     ap.add_argument("--command", default=None, help="the ncu command that made the report (kept in the JSON)")
     ap.add_argument("--json", default=None, help="profiles/ncu_traffic.json to update")
     ap.add_argument("--md", default=None, help="file to append the counter table to ('-' = stdout)")
+    ap.add_argument("--sum", action="store_true",
+                    help="the report holds the launches of ONE step (a catalogue beyond one constant-bank slot-load runs "
+                         "as several launches that carry partial sums): the JSON entry sums bytes and durations over them")
     a = ap.parse_args()
     hdr, units, rows = read_rows(sys.stdin)
     col = {h: i for i, h in enumerate(hdr)}
@@ -95,10 +98,15 @@ def main():
         rec.setdefault("what", "dram__bytes_read.sum / dram__bytes_write.sum (bytes) per launch of each mode's dominant kernel, "
                                "from `ncu --set full` captures; written by paper_1902_03252_b200/ncu_extract.py")
         rec["commit"] = a.commit or rec.get("commit")
+        over = cand if a.sum else [row]
+
+        def tot(name):
+            return sum(num(r, name) or 0.0 for r in over)
         rec["captures"]["%s/%s" % (a.workload, a.mode)] = {
             "kernel": row[col["Kernel Name"]].split("(")[0].strip(), "launches_in_report": len(cand),
-            "dram_bytes_read": num(row, "dram__bytes_read.sum"), "dram_bytes_write": num(row, "dram__bytes_write.sum"),
-            "duration_ns_under_ncu": num(row, "gpu__time_duration.sum"), "commit": a.commit, "command": a.command}
+            "launches_summed": len(over),
+            "dram_bytes_read": tot("dram__bytes_read.sum"), "dram_bytes_write": tot("dram__bytes_write.sum"),
+            "duration_ns_under_ncu": tot("gpu__time_duration.sum"), "commit": a.commit, "command": a.command}
         json.dump(rec, open(a.json, "w"), indent=1, sort_keys=True)
     if a.md:
         out = sys.stdout if a.md == "-" else open(a.md, "a")
