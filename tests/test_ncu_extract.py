@@ -33,3 +33,20 @@ def test_extract_json_and_markdown(tmp_path):
     r = subprocess.run([sys.executable, "-m", "paper_1902_03252_b200.ncu_extract", "--kernel", "lt_flag_kernel",
                         "--workload", "w", "--mode", "mixed", "--json", str(js)], input=CSV, capture_output=True, text=True, cwd=ROOT)
     assert r.returncode == 0 and set(json.load(open(js))["captures"]) == {"cfg3_4096x4096_1000/fp64", "w/mixed"}
+    # --sum: the launches of one step (a catalogue beyond one constant-bank slot-load) are added up
+    r = subprocess.run([sys.executable, "-m", "paper_1902_03252_b200.ncu_extract", "--sum", "--kernel", "lt_grad_f64_kernel",
+                        "--workload", "s", "--mode", "fp64", "--json", str(js)], input=CSV, capture_output=True, text=True, cwd=ROOT)
+    e = json.load(open(js))["captures"]["s/fp64"]
+    assert r.returncode == 0 and e["launches_summed"] == 2 and e["dram_bytes_read"] == 104867 and e["dram_bytes_write"] == 268435476
+    assert e["duration_ns_under_ncu"] == 68000500
+
+
+def test_bench_reports_the_step_traffic_of_the_constant_bank_kernels():
+    """profiles/ncu_traffic.json as committed: the fp64 headline entry is the sum over the launches of one step and says so."""
+    sys.path.insert(0, ROOT)
+    import bench
+    t = bench.ncu_traffic("cfg3_4096x4096_1000", "fp64")
+    assert t is not None and t["launches_summed"] == 3 and "const" in t["kernel"] and "note" in t
+    assert t["bytes"] == t["read"] + t["write"] > 3 * 4096 * 4096 * 16 * 0.7      # three writes of the map (+ two re-reads)
+    s = bench.ncu_traffic("sie_paper_6730x6730_702", "fp64")
+    assert s is not None and "launches_summed" not in s
