@@ -64,8 +64,8 @@ MODEL_TYPE = {"dpie": "LtDpieModel", "sie": "LtSieModel", "nfw": "LtNfwModel"}
 
 
 def kernel_name(model, mode):
-    """The dominant kernel of a step (the 4-pixel launch; the dPIE fp64 kernels read their records from the constant bank)."""
-    const = "_const" if model == "dpie" else ""
+    """The dominant kernel of a step (the 4-pixel launch; the dPIE and SIE fp64 kernels read their records from the constant bank)."""
+    const = "_const" if model in ("dpie", "sie") else ""
     return {"fp64": "lt_grad_f64%s_kernel<%s>" % (const, MODEL_TYPE[model]),
             "fp32": "lt_grad_f32_kernel<%s, 4, 3>" % MODEL_TYPE[model],
             "mixed": "lt_grad_quads_f64%s_kernel<%s>" % (const, MODEL_TYPE[model])}[mode]
@@ -82,7 +82,7 @@ def kernel_name(model, mode):
 # per interaction max(2, source words / 2) summed over the loop's pipe instructions.
 PIPE_FLOOR = {("dpie", "fp64"): ("fp64", 60.75, 2.0, 128.5), ("dpie", "mixed"): ("fp64", 60.75, 2.0, 128.5),
               ("dpie", "fp32"): ("fp32 fma (packed pairs)", 20.0, 2.0, 44.5),
-              ("sie", "fp64"): ("fp64", 12.75, 2.0, 30.5), ("sie", "mixed"): ("fp64", 12.75, 2.0, 30.5),
+              ("sie", "fp64"): ("fp64", 12.75, 2.0, 28.5), ("sie", "mixed"): ("fp64", 12.75, 2.0, 28.5),
               ("sie", "fp32"): ("xu (MUFU.RSQ)", 1.0, 8.0, 9.25)}
 # dram__bytes_{read,write}.sum per launch of the dominant kernels, written by the ncu recipe of profiles/README.md
 NCU_TRAFFIC_JSON = os.path.join(ROOT, "profiles", "ncu_traffic.json")

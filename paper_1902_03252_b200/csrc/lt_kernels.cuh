@@ -184,6 +184,38 @@ lt_grad_f64_kernel(const typename M::template Rec<double>::type* __restrict__ le
 #define LT_CONST_SLOT_BYTES 57344
 __constant__ double2 lt_const_slot[LT_CONST_SLOT_BYTES / 16];
 
+// The lens loop of the constant-bank kernels for four pixels of a row: M::kConstGroup lenses per iteration.  The records
+// of a group are all requested at its top (LDCU into uniform registers: no vector register is spent on them), so a short
+// loop body -- the SIE's 66 instructions per lens -- does not wait for its record at every lens; the dPIE body is long
+// enough alone and is not grouped (grouped, its loop outgrows the instruction cache: config 2 +7 % at 8 per group).
+template <class M>
+__device__ __forceinline__ void lt_const_lens_loop(const typename M::template Rec<double>::type* cl, int n_lens, double t2,
+                                                   const double (&t1)[4], const LtTables<double>& tab, double (&G1)[4],
+                                                   double (&G2)[4]) {
+  typedef typename M::template Rec<double>::type Rec;
+  constexpr int GROUP = M::kConstGroup;
+  int k = 0;
+  if constexpr (GROUP > 1) {
+#pragma unroll 1
+    for (; k + GROUP <= n_lens; k += GROUP) {
+#pragma unroll
+      for (int u = 0; u < GROUP; ++u) {
+        const Rec& L = cl[k + u];
+        const auto row = M::template row_abs<double>(t2, L);
+#pragma unroll
+        for (int p = 0; p < 4; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
+      }
+    }
+  }
+#pragma unroll 1
+  for (; k < n_lens; ++k) {
+    const Rec& L = cl[k];
+    const auto row = M::template row_abs<double>(t2, L);
+#pragma unroll
+    for (int p = 0; p < 4; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
+  }
+}
+
 // INPLACE: `acc` is a flag and the partial sums are read from `out` itself (device output); else `acc` is the buffer they
 // are read from (null: start from zero) -- two instantiations because the in-place form compiles to the faster loop
 template <class M, bool INPLACE>
@@ -219,13 +251,7 @@ lt_grad_f64_const_kernel(const LtTables<double>* __restrict__ tables, int n_lens
         G2[p] = g.y;
       }
     }
-#pragma unroll 1
-    for (int k = 0; k < n_lens; ++k) {
-      const Rec& L = cl[k];
-      const auto row = M::template row_abs<double>(t2, L);
-#pragma unroll
-      for (int p = 0; p < PPT; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
-    }
+    lt_const_lens_loop<M>(cl, n_lens, t2, t1, tab, G1, G2);
     if (j < ny) {
 #pragma unroll
       for (int p = 0; p < PPT; ++p) {
@@ -595,13 +621,7 @@ lt_grad_quads_f64_const_kernel(const LtTables<double>* __restrict__ tables, int 
         G2[p] = v.y;
       }
     }
-#pragma unroll 1
-    for (int k = 0; k < n_lens; ++k) {
-      const Rec& L = cl[k];
-      const auto row = M::template row_abs<double>(t2, L);
-#pragma unroll
-      for (int p = 0; p < 4; ++p) M::template interact_abs<double, true>(t1[p], row, L, tab, G1[p], G2[p]);
-    }
+    lt_const_lens_loop<M>(cl, n_lens, t2, t1, tab, G1, G2);
 #pragma unroll
     for (int p = 0; p < 4; ++p)
       if (keep[p]) out[p0 + p] = make_double2(G1[p], G2[p]);

@@ -175,3 +175,32 @@ def test_host_buffer_entry_point(env):
         lt.lt_gradient_grid_sie_host(hL, W.x_min, W.y_min, W.dx, W.nx, W.ny, mode, hout, ws)
         torch.cuda.synchronize()
         assert np.array_equal(hout.numpy(), _gpu(torch, lt, W, mode))
+
+
+@pytest.mark.parametrize("n_lens,nx,ny", [(37, 1400, 650), (702, 1500, 700), (1300, 1111, 600)])
+def test_sie_records_from_the_constant_bank_give_the_same_bits(env, n_lens, nx, ny):
+    """The SIE fp64 kernels (grid and quad) read their 48-byte records from __constant__ memory into uniform registers,
+    eight lenses per iteration plus a lens-by-lens rest (37 = 4 groups + 5; 1300 records = two slot-loads that continue each
+    other's sums); lt_set_tuning bit 5 keeps them in shared memory.  Same operations in the same order: fp64 and mixed maps
+    bit-equal, through the host entry point too."""
+    torch, lt, S, O = env
+    rng = np.random.default_rng(500 + n_lens)
+    L = np.stack([rng.uniform(-60, 60, n_lens), rng.uniform(-25, 25, n_lens), rng.uniform(0.0, 0.15, n_lens),
+                  rng.uniform(0.0, np.pi, n_lens), rng.uniform(0.05, 0.3, n_lens)], axis=1)
+    L[0, 4], L[1, 4] = 28.8, 14.1
+    W = workloads.Workload("sie_const", L, -60.0, -25.0, 0.085, nx, ny, 0)
+    res = {}
+    for bit in (0, 32):
+        try:
+            lt.lt_set_tuning(single_launch=bit)
+            res[bit] = (_gpu(torch, lt, W, lt.LT_FP64), _gpu(torch, lt, W, lt.LT_MIXED, mixed=SIE_MIXED))
+        finally:
+            lt.lt_set_tuning()
+    assert np.array_equal(res[0][0], res[32][0]) and np.array_equal(res[0][1], res[32][1])
+    assert np.isfinite(res[0][0]).all()
+    hL = torch.from_numpy(L).pin_memory()
+    hout = torch.full((ny, nx, 2), float("nan"), dtype=torch.float64).pin_memory()
+    wsh = lt.alloc_workspace(n_lens, nx, ny, lt.LT_FP64, host=True)
+    lt.lt_gradient_grid_sie_host(hL, W.x_min, W.y_min, W.dx, nx, ny, lt.LT_FP64, hout, wsh)
+    torch.cuda.synchronize()
+    assert np.array_equal(hout.numpy(), res[0][0])
