@@ -160,6 +160,7 @@ struct LtDpieModel {
   static constexpr bool kPacked32 = true;      // the fp32 grid kernel evaluates two pixels per instruction (interact_lens_x2)
   static constexpr bool kConstRecords = true;  // fp64 kernels: records from the constant bank where the call allows it (+3 % at config 3)
   static constexpr int kConstGroup = 1;        // lenses per iteration of the constant-bank loops (lt_kernels.cuh: lt_const_lens_loop)
+  static constexpr int kGroup32 = 2;           // lenses per iteration of the packed fp32 grid kernel
 #if defined(__CUDACC__)
   static __device__ __forceinline__ void interact_lens_x2(const lt_f2 X, const lt_f2 Y, const LtLens<float>& L,
                                                           const LtTables2& tab, lt_f2& G1, lt_f2& G2) {
@@ -208,6 +209,7 @@ struct LtSieModel {
   // not hidden (3 % slower than shared memory), eight lenses per iteration are 5 % faster (SIE benchmark 26.8 -> 25.4 ms)
   static constexpr bool kConstRecords = true;
   static constexpr int kConstGroup = 8;
+  static constexpr int kGroup32 = 8;
 #if defined(__CUDACC__)
   static __device__ __forceinline__ void interact_sky_x2(const lt_f2 d1, const LtSieRow<float>& r, const LtSieLens<float>& L,
                                                          const LtTables2&, lt_f2& G1, lt_f2& G2) {
@@ -243,6 +245,7 @@ struct LtNfwModel {
   static constexpr bool kPacked32 = false;
   static constexpr bool kConstRecords = false; // measured: -2 % fp64, +0.5 % mixed (profiles/r02_fp64_pipe_diagnostics.md section 13)
   static constexpr int kConstGroup = 1;
+  static constexpr int kGroup32 = 1;
   static LT_HD bool valid(const Raw& r) { return lt_nfw_valid(r); }
   static LT_HD void pack(const Raw& r, LtNfwLens<double>& L) { lt_pack_nfw(r, L); }
   static LT_HD void poison(LtNfwLens<double>& L) { lt_poison_nfw(L); }
