@@ -401,7 +401,9 @@ def test_calibration_tool_on_small_workloads(env):
         assert tc["calibrated_rule"]["violating_and_missed"] == 0
         assert tc["calibrated_rule"]["flagged_fraction"] <= tc["criterion"]["flagged_fraction"] + 1e-12
         assert tc["implied_m_max_no_patches"] > 3.26
-        assert pl["sp_error_arcsec"]["max"] >= tc["sp_error_arcsec"]["max"]
+        # cored dPIE: both versions carry the rounding of the sum and differ by a few per cent either way (DESIGN.md
+        # section 13); the singular SIE is where the plain version's coordinate rounding shows
+        assert pl["sp_error_arcsec"]["max"] >= (1.0 if model == "sie" else 0.8) * tc["sp_error_arcsec"]["max"]
         if model == "sie":                                     # the paper's own case: SIS direction theta / R at the centres
             near = list(pl["max_sp_error_by_distance_px"].values())
             assert max(near[:3]) > 3 * max(near[5:])           # plain SP: worst within a few pixels of a centre
