@@ -81,7 +81,7 @@ def kernel_name(model, mode):
 # delivers two 32-bit source reads per lane and cycle: lt_peak_probe 3 / 4, `peak_probe` below) --
 # per interaction max(2, source words / 2) summed over the loop's pipe instructions.
 PIPE_FLOOR = {("dpie", "fp64"): ("fp64", 60.75, 2.0, 128.5), ("dpie", "mixed"): ("fp64", 60.75, 2.0, 128.5),
-              ("dpie", "fp32"): ("fp32 fma (packed pairs)", 20.0, 2.0, 44.5),
+              ("dpie", "fp32"): ("fp32 fma (packed pairs)", 20.0, 2.0, 43.5),
               ("sie", "fp64"): ("fp64", 12.75, 2.0, 28.5), ("sie", "mixed"): ("fp64", 12.75, 2.0, 28.5),
               ("sie", "fp32"): ("xu (MUFU.RSQ)", 1.0, 8.0, 9.25)}
 # dram__bytes_{read,write}.sum per launch of the dominant kernels, written by the ncu recipe of profiles/README.md
