@@ -508,3 +508,34 @@ def test_call_is_capturable_in_a_cuda_graph(env):
         if mode == lt.LT_FP64:
             assert torch.allclose(out, 2.0 * expect, rtol=1e-13, atol=0)
         L.copy_(torch.from_numpy(W.lenses).cuda())
+
+
+@pytest.mark.parametrize("n_lens,chunk", [(1, 0), (7, 0), (9, 5), (33, 0), (64, 7)])
+def test_fp32_lens_groups_and_remainders(env, n_lens, chunk):
+    """The packed fp32 kernels take several lenses per iteration (dPIE 2, SIE 8) plus a lens-by-lens rest, per shared-memory
+    chunk: catalogue sizes and chunk lengths (lt_set_tuning) that leave every remainder, against the oracles (1e-5), and the
+    same bits whatever the chunking."""
+    torch, lt, O = env
+    from oracle import lt_oracle_sie as S
+    nx, ny = 300, 41
+    Wd = workloads.Workload("grp", workloads.random_catalogue(900 + n_lens, n_lens, L=40.0), -40.0, -6.0, 0.27, nx, ny, 0)
+    rng = np.random.default_rng(950 + n_lens)
+    Ls = np.stack([rng.uniform(-40, 40, n_lens), rng.uniform(-6, 6, n_lens), rng.uniform(0.0, 0.15, n_lens),
+                   rng.uniform(0.0, np.pi, n_lens), rng.uniform(0.5, 3.0, n_lens)], axis=1)
+    refd = O.gradient_grid(Wd.lenses, Wd.x_min, Wd.y_min, Wd.dx, nx, ny)
+    refs = S.gradient_grid(Ls, Wd.x_min, Wd.y_min, Wd.dx, nx, ny)
+    base = None
+    for ch in sorted({0, chunk}):
+        try:
+            lt.lt_set_tuning(chunk32=ch)
+            d = _gpu_map(torch, lt, Wd, lt.LT_FP32)
+            s = lt.lt_gradient_grid_sie(torch.from_numpy(Ls).cuda(), Wd.x_min, Wd.y_min, Wd.dx, nx, ny, lt.LT_FP32)
+            torch.cuda.synchronize()
+            s = s.cpu().numpy()
+        finally:
+            lt.lt_set_tuning()
+        assert _err(d, refd) < TOL_F32 and _err(s, refs) < TOL_F32, (n_lens, ch, _err(d, refd), _err(s, refs))
+        if base is None:
+            base = (d, s)
+        else:
+            assert np.array_equal(d, base[0]) and np.array_equal(s, base[1])
